@@ -1,0 +1,143 @@
+/*
+ * qsgw_oracle.c -- TEST INFRASTRUCTURE, not product code.
+ *
+ * Plain, slow, obviously-correct CPU FP64 statement of what the qsGW correlation
+ * self-energy path computes, written from the paper's equations (arxiv 2210.17093,
+ * /root/reference/PAPER.md) in its resolution-of-identity (RI) form.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * build, load or call this file.  It shares no code, header, table or helper with the
+ * CUDA path under paper_2210_17093_b200/csrc/, and neither includes the other.
+ *
+ * What it computes (Eqs. (17)-(19); RI remark PAPER.md:120):
+ *
+ *   1. V[P][s]    = sum_{i<o} sum_{a>=o} B[P][i][a] * Z[i*v + (a-o)][s]        first half of Eq. (18)
+ *   2. w[s][p][m] = sqrt(2) * sum_P B[P][p][m] * V[P][s]                        second half of Eq. (18)
+ *   3. Sigma[p][q] = 1/2 * sum_m sum_s w[s][p][m] w[s][q][m] (D(m,s,eps[p]) + D(m,s,eps[q]))
+ *                                                                              Eq. (17) put into Eq. (19)
+ *      D(m,s,omega) = occ[m]     * x1/(x1*x1 + eta*eta),  x1 = omega - eps[m] + Omega[s]
+ *                   + (1-occ[m]) * x2/(x2*x2 + eta*eta),  x2 = omega - eps[m] - Omega[s]
+ *      (real part of the two terms of Eq. (17); Re[1/(x -+ i eta)] = x/(x^2+eta^2)).
+ *
+ * Readings of the paper taken here are the ones listed in DESIGN.md ("Readings"):
+ * the (ia) composite index is i*v + (a-o) with a fastest; closed shell, one spin channel,
+ * prefactor sqrt(2) on w; eta is a finite positive input; one array eps serves as the
+ * poles eps[m] and as the evaluation points eps[p], eps[q]; p, q, m run over all N states.
+ * The oracle does NOT assume B symmetric in its last two indices: it reads B[P][p][m]
+ * literally.
+ *
+ * Layouts (row-major C arrays): B[naux][N][N], Z[o*v][ldz], V[naux][ldv], Sigma[N][N].
+ *
+ * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): hand-solved two-state case with
+ * exact rationals (tests/golden/two_state_single_pole.txt), literal complex evaluation of
+ * Eq. (17), non-RI 4-index brute force of Eq. (18) on tiny inputs, symmetry, exact
+ * power-of-two scaling, additivity over poles, eta->0 limit, null case, separable closed
+ * form, permutation invariances, diagonal == G0W0 expression.
+ *
+ * Floating point: products and the P-, ia- and m-sums are plain double; the running sum
+ * over poles s of step 3 is kept in long double so that the oracle's own rounding is far
+ * below the 1e-9 parity budget.
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int qsgw_oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/* D(m,s,omega): real part of the two Lehmann terms of Eq. (17). */
+double qsgw_oracle_D(double occ_m, double eps_m, double Omega_s, double omega, double eta) {
+  double x1 = omega - eps_m + Omega_s;
+  double x2 = omega - eps_m - Omega_s;
+  return occ_m * (x1 / (x1 * x1 + eta * eta)) + (1.0 - occ_m) * (x2 / (x2 * x2 + eta * eta));
+}
+
+/* Step 1, first half of Eq. (18) after (pm|ia) = sum_P B^P_pm B^P_ia (RI):
+ *   V[P][s] = sum_i sum_a B[P][i][a] * Z[i*v + (a-o)][s],   i < o <= a < N,  s in [0, n_pole). */
+void qsgw_oracle_pole_weights(int N, int o, int naux, int64_t n_pole, const double *B, const double *Z,
+                              int64_t ldz, double *V, int64_t ldv) {
+  const int v = N - o;
+#pragma omp parallel for schedule(static)
+  for (int P = 0; P < naux; ++P) {
+    double *Vrow = V + (size_t)P * ldv;
+    for (int64_t s = 0; s < n_pole; ++s) Vrow[s] = 0.0;
+    for (int i = 0; i < o; ++i) {
+      for (int a = o; a < N; ++a) {
+        const double b = B[((size_t)P * N + i) * N + a];
+        const double *Zrow = Z + ((size_t)i * v + (a - o)) * ldz;
+        for (int64_t s = 0; s < n_pole; ++s) Vrow[s] += b * Zrow[s];
+      }
+    }
+  }
+}
+
+/* Step 2, second half of Eq. (18) for ONE pole s and the listed rows p (rows == NULL: all p):
+ *   w[r][m] = sqrt(2) * sum_P B[P][p_r][m] * V[P][s]. */
+void qsgw_oracle_residues(int N, int naux, const double *B, const double *V, int64_t ldv, int64_t s,
+                          int n_rows, const int *rows, double *w) {
+  const double sqrt2 = sqrt(2.0);
+#pragma omp parallel for schedule(static)
+  for (int r = 0; r < n_rows; ++r) {
+    const int p = rows ? rows[r] : r;
+    double *wr = w + (size_t)r * N;
+    for (int m = 0; m < N; ++m) wr[m] = 0.0;
+    for (int P = 0; P < naux; ++P) {
+      const double vps = V[(size_t)P * ldv + s];
+      const double *Brow = B + ((size_t)P * N + p) * N;
+      for (int m = 0; m < N; ++m) wr[m] += Brow[m] * vps;
+    }
+    for (int m = 0; m < N; ++m) wr[m] *= sqrt2;
+  }
+}
+
+/* Steps 1-3 restricted to the output rows/columns listed in `states` (n_states entries; NULL: all N
+ * states, n_states = N) and to the poles [0, n_pole) of the arrays handed in:
+ *   Sigma[r][c] = 1/2 sum_m sum_s w[s][p_r][m] w[s][p_c][m] (D(m,s,eps[p_r]) + D(m,s,eps[p_c]))
+ * Sigma is n_states x n_states, row-major.  Loop order: s outermost; w^s is built, used, discarded
+ * (w is never held whole).  Returns 0, or -1 on allocation failure / bad arguments. */
+int qsgw_oracle_sigma(int N, int o, int naux, int64_t n_pole, const double *B, const double *eps,
+                      const double *occ, const double *Omega, const double *Z, int64_t ldz, double eta,
+                      int n_states, const int *states, double *Sigma) {
+  if (N < 2 || o < 1 || o >= N || naux < 1 || n_pole < 1 || ldz < n_pole || !(eta > 0.0)) return -1;
+  if (!states) n_states = N;
+  if (n_states < 1) return -1;
+  const size_t nS = (size_t)n_states;
+  double *V = (double *)malloc(sizeof(double) * (size_t)naux * (size_t)n_pole);
+  double *w = (double *)malloc(sizeof(double) * nS * N);
+  double *Dm = (double *)malloc(sizeof(double) * nS * N);
+  long double *acc = (long double *)malloc(sizeof(long double) * nS * nS);
+  if (!V || !w || !Dm || !acc) { free(V); free(w); free(Dm); free(acc); return -1; }
+  for (size_t k = 0; k < nS * nS; ++k) acc[k] = 0.0L;
+
+  qsgw_oracle_pole_weights(N, o, naux, n_pole, B, Z, ldz, V, n_pole);            /* step 1 */
+
+  for (int64_t s = 0; s < n_pole; ++s) {
+    qsgw_oracle_residues(N, naux, B, V, n_pole, s, n_states, states, w);        /* step 2 */
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < n_states; ++r) {                                         /* D(m,s,eps[p_r]) */
+      const int p = states ? states[r] : r;
+      for (int m = 0; m < N; ++m) Dm[(size_t)r * N + m] = qsgw_oracle_D(occ[m], eps[m], Omega[s], eps[p], eta);
+    }
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < n_states; ++r) {                                         /* step 3, this pole */
+      for (int c = 0; c < n_states; ++c) {
+        double t = 0.0;
+        for (int m = 0; m < N; ++m)
+          t += w[(size_t)r * N + m] * w[(size_t)c * N + m] * (Dm[(size_t)r * N + m] + Dm[(size_t)c * N + m]);
+        acc[(size_t)r * nS + c] += 0.5L * (long double)t;
+      }
+    }
+  }
+  for (size_t k = 0; k < nS * nS; ++k) Sigma[k] = (double)acc[k];
+  free(V); free(w); free(Dm); free(acc);
+  return 0;
+}

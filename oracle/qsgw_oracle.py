@@ -1,0 +1,131 @@
+"""ctypes binding of oracle/qsgw_oracle.c (plain C FP64 loops) -- TEST INFRASTRUCTURE.
+
+The arithmetic lives in qsgw_oracle.c (each function cites the passage of
+/root/reference/PAPER.md it follows: Eqs. (17)-(19), in RI form).
+This file only compiles that C file with gcc, marshals numpy arrays, and returns numpy
+arrays.  It imports nothing from the CUDA product package.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "qsgw_oracle.c")
+_LIB = os.path.join(_HERE, "libqsgw_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+
+def build_library(force: bool = False) -> str:
+    """Compile qsgw_oracle.c -> libqsgw_oracle.so with gcc (-O2 -fopenmp); returns the path."""
+    with _lock:
+        stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
+        if force or stale:
+            tmp = _LIB + f".tmp{os.getpid()}"
+            cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-o", tmp, _SRC, "-lm"]
+            subprocess.run(cmd, check=True)
+            os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build_library())
+        dp = ctypes.POINTER(ctypes.c_double)
+        ip = ctypes.POINTER(ctypes.c_int)
+        i64 = ctypes.c_int64
+        lib.qsgw_oracle_num_threads.restype = ctypes.c_int
+        lib.qsgw_oracle_D.restype = ctypes.c_double
+        lib.qsgw_oracle_D.argtypes = [ctypes.c_double] * 5
+        lib.qsgw_oracle_pole_weights.restype = None
+        lib.qsgw_oracle_pole_weights.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i64, dp, dp, i64, dp, i64]
+        lib.qsgw_oracle_residues.restype = None
+        lib.qsgw_oracle_residues.argtypes = [ctypes.c_int, ctypes.c_int, dp, dp, i64, i64, ctypes.c_int, ip, dp]
+        lib.qsgw_oracle_sigma.restype = ctypes.c_int
+        lib.qsgw_oracle_sigma.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i64, dp, dp, dp, dp, dp, i64,
+                                          ctypes.c_double, ctypes.c_int, ip, dp]
+        _lib = lib
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _f64(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if shape is not None and a.shape != tuple(shape):
+        raise ValueError(f"expected shape {tuple(shape)}, got {a.shape}")
+    return a
+
+
+def num_threads() -> int:
+    """OpenMP threads the oracle will use (its `cores` figure when timed as the CPU baseline)."""
+    return int(_load().qsgw_oracle_num_threads())
+
+
+def D(occ_m: float, eps_m: float, Omega_s: float, omega: float, eta: float) -> float:
+    """D(m,s,omega) of SURVEY 8(c): real part of the two terms of Eq. (17)."""
+    return float(_load().qsgw_oracle_D(occ_m, eps_m, Omega_s, omega, eta))
+
+
+def pole_weights(B, Z, n_occ: int):
+    """Step 1: V[P,s] = sum_ia B[P,i,a] Z[ia,s]  (first half of Eq. (18), RI form)."""
+    B = _f64(B)
+    naux, N, _ = B.shape
+    Z = _f64(Z, (n_occ * (N - n_occ), np.shape(Z)[1]))
+    n_pole = Z.shape[1]
+    V = np.empty((naux, n_pole))
+    _load().qsgw_oracle_pole_weights(N, n_occ, naux, n_pole, _dp(B), _dp(Z), n_pole, _dp(V), n_pole)
+    return V
+
+
+def residues(B, V, s: int, rows=None):
+    """Step 2 for one pole s: w[r,m] = sqrt(2) sum_P B[P,p_r,m] V[P,s]  (Eq. (18))."""
+    B = _f64(B)
+    naux, N, _ = B.shape
+    V = _f64(V)
+    if rows is None:
+        n_rows, rp, keep = N, None, None
+    else:
+        keep = np.ascontiguousarray(rows, dtype=np.int32)
+        n_rows, rp = len(keep), keep.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+    w = np.empty((n_rows, N))
+    _load().qsgw_oracle_residues(N, naux, _dp(B), _dp(V), V.shape[1], int(s), n_rows, rp, _dp(w))
+    return w
+
+
+def sigma(B, eps, occ, Omega, Z, eta: float, n_occ: int, states=None):
+    """Steps 1-3: Sigma (Eqs. (17)-(19)) for the poles handed in.
+
+    ``states`` (optional list of MO indices) restricts the OUTPUT to those rows/columns;
+    all internal sums (ia, P, m, s) still run over their full ranges.
+    """
+    B = _f64(B)
+    naux, N, N2 = B.shape
+    if N != N2:
+        raise ValueError("B must be [naux, N, N]")
+    eps = _f64(eps, (N,))
+    occ = _f64(occ, (N,))
+    Omega = _f64(Omega)
+    n_pole = Omega.shape[0]
+    Z = _f64(Z, (n_occ * (N - n_occ), n_pole))
+    if states is None:
+        n_states, sp, keep = N, None, None
+    else:
+        keep = np.ascontiguousarray(states, dtype=np.int32)
+        if keep.min() < 0 or keep.max() >= N:
+            raise ValueError("states out of range")
+        n_states, sp = len(keep), keep.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+    out = np.empty((n_states, n_states))
+    rc = _load().qsgw_oracle_sigma(N, n_occ, naux, n_pole, _dp(B), _dp(eps), _dp(occ), _dp(Omega), _dp(Z),
+                                   n_pole, float(eta), n_states, sp, _dp(out))
+    if rc != 0:
+        raise RuntimeError(f"qsgw_oracle_sigma failed with {rc}")
+    return out
