@@ -1,0 +1,154 @@
+/*
+ * qsgw_sigma.h -- C ABI of the B200 (sm_100a) qsGW correlation self-energy build.
+ *
+ * What the library computes (arxiv 2210.17093; citations are lines of /root/reference/PAPER.md):
+ * the full off-diagonal "mode A" quasiparticle self-consistent GW correlation self-energy
+ * matrix of Eq. (19), with Sigma^GW(omega) the Lehmann sum of Eq. (17)
+ * and the residues w of Eq. (18), in resolution-of-identity
+ * form, (pm|ia) = sum_P B^P_pm B^P_ia (RI remark):
+ *
+ *   stage 1   V[P][s]    = sum_{i<o<=a} B[P][i][a] * Z[i*v+(a-o)][s]                  (Eq. 18, first half)
+ *   stage 2   w[s][p][m] = sqrt(2) * sum_P B[P][p][m] * V[P][s]                      (Eq. 18, second half)
+ *   stage 3   T[p][q]    = sum_m sum_s ( w[s][p][m] * D(m,s,eps[p]) ) * w[s][q][m]   (Eq. 17 at omega = eps[p])
+ *   epilogue  Sigma[p][q] = 1/2 ( T[p][q] + T[q][p] )                                (Eq. 19)
+ *   D(m,s,omega) = occ[m]     * x1/(x1^2+eta^2),  x1 = omega - eps[m] + Omega[s]
+ *                + (1-occ[m]) * x2/(x2^2+eta^2),  x2 = omega - eps[m] - Omega[s]     (real part of Eq. 17's terms)
+ *
+ * All arithmetic is FP64.  Every step runs in hand-written CUDA kernels (FP64 tensor-core DMMA
+ * tiles); there is no CPU fallback: without a CUDA device every entry point that needs one
+ * returns QSGW_SIGMA_ERR_CUDA.
+ *
+ * Conventions
+ *   - All arrays are dense, row-major (C order), FP64.
+ *   - "device" pointers are CUDA device pointers valid on the device the plan was created on;
+ *     "host" pointers are ordinary host memory (pinned memory makes the copies faster, it is not required).
+ *   - The caller owns every array it passes.  The plan owns its workspace (packed copies of B,
+ *     V, the w chunk, split-K partial tiles), allocated in qsgw_sigma_create, freed in
+ *     qsgw_sigma_destroy.  No build call allocates device memory.
+ *   - Device entry points are asynchronous on the plan's stream: inputs must stay alive and
+ *     unmodified, and Sigma must not be read, until the stream has been synchronised.
+ *   - Return value: QSGW_SIGMA_OK (0) or a negative qsgw_sigma_status.  No exception or abort
+ *     crosses the ABI.  qsgw_sigma_last_error(plan) gives a message for the last failure.
+ *   - Preconditions that would need a look at device data are NOT checked:
+ *     B[P][p][q] == B[P][q][p] (real orbitals), occ[m] in [0,1], Omega[s] > 0.
+ */
+#ifndef QSGW_SIGMA_H
+#define QSGW_SIGMA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qsgw_sigma_plan qsgw_sigma_plan; /* opaque */
+
+typedef enum qsgw_sigma_status {
+  QSGW_SIGMA_OK = 0,
+  QSGW_SIGMA_ERR_INVALID_ARG = -1, /* null pointer, size out of range, eta <= 0, call out of sequence */
+  QSGW_SIGMA_ERR_ALLOC = -2,       /* workspace allocation failed */
+  QSGW_SIGMA_ERR_CUDA = -3         /* a CUDA call failed (no device, launch error, ...) */
+} qsgw_sigma_status;
+
+/* Per-stage device times of the builds since the last reset, measured with CUDA events on the plan's
+ * stream around every kernel launch (only while profiling is on; see qsgw_sigma_set_profiling). */
+typedef struct qsgw_sigma_stats {
+  double ms_pack;     int64_t launches_pack;     /* symmetric-pair pack of B + transposed ov block   */
+  double ms_stage1;   int64_t launches_stage1;   /* V = B_ov * Z                      (DMMA GEMM)      */
+  double ms_stage2;   int64_t launches_stage2;   /* w chunk = sqrt(2) B^T V           (DMMA GEMM)      */
+  double ms_stage3;   int64_t launches_stage3;   /* T += (w.D) w^T                    (fused DMMA)     */
+  double ms_epilogue; int64_t launches_epilogue; /* split-K reduce + symmetrise                         */
+  int64_t builds;                                /* number of qsgw_sigma_finish calls                  */
+  int64_t poles;                                 /* poles processed                                    */
+} qsgw_sigma_stats;
+
+/*
+ * Create a plan for problems with n_mo molecular orbitals (N), of which the first n_occ are the
+ * occupied ones that define the (ia) block of stage 1, n_aux auxiliary functions, and at most
+ * n_pole_max poles per qsgw_sigma_build / qsgw_sigma_add_poles call.
+ *   s_block     : poles per internal w chunk (the config's "s-block"); 0 = library default (2048).
+ *                 w is only ever materialised for one chunk: workspace holds n_mo*n_mo*s_block doubles.
+ *   cuda_stream : a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream), or NULL for the
+ *                 legacy default stream.  All work of this plan is enqueued on it.
+ * Errors: INVALID_ARG if plan == NULL, n_mo < 2, n_occ not in [1, n_mo-1], n_aux < 1, n_pole_max < 1,
+ * s_block < 0; ALLOC if the workspace does not fit; CUDA if no usable device.
+ */
+int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, int64_t n_pole_max,
+                      int s_block, void *cuda_stream);
+
+/*
+ * One-shot build: Sigma (Eq. 19) from all n_pole poles handed in.  Equivalent to
+ * qsgw_sigma_begin + qsgw_sigma_add_poles + qsgw_sigma_finish.
+ *   B      device [n_aux][n_mo][n_mo]   RI factors in the MO basis, symmetric in the last two indices
+ *   eps    device [n_mo]                QP energies (Ha): the poles eps[m] AND the evaluation points eps[p], eps[q]
+ *   occ    device [n_mo]                occupations f_m in [0,1] (0 or 1)
+ *   Omega  device [n_pole]              RPA excitation energies (Ha), > 0                       (Eq. 12)
+ *   Z      device [n_occ*n_virt][ldz]   X+Y of Eq. (18); row i*n_virt + (a - n_occ), column s
+ *   ldz    leading dimension of Z, >= n_pole (a pole sub-range is Z + s0, Omega + s0 with the full ldz)
+ *   n_pole poles in this call, 1 <= n_pole <= n_pole_max
+ *   eta    > 0 (Ha)
+ *   Sigma  device [n_mo][n_mo]          OVERWRITTEN; bit-symmetric (Sigma[p][q] == Sigma[q][p])
+ * Because Eq. (17) is a plain sum over s, Sigma of a set of poles is the sum of the Sigmas of any
+ * partition of it.
+ */
+int qsgw_sigma_build(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ,
+                     const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
+                     double *Sigma);
+
+/*
+ * Streaming form, for pole sets that are produced or uploaded range by range (Z of the xl config is
+ * 130 GB): begin once per Sigma, add any number of pole ranges, finish once.
+ *   qsgw_sigma_begin     packs B (symmetric pairs + transposed ov block), keeps eps/occ/eta, zeroes the accumulators.
+ *                        B, eps, occ must stay valid until qsgw_sigma_finish has completed on the stream.
+ *   qsgw_sigma_add_poles stages 1-3 for the poles handed in, accumulated into the plan's split-K partial tiles.
+ *   qsgw_sigma_finish    fixed-order reduction of the partial tiles and Sigma = (T + T^T)/2.
+ * INVALID_ARG if called out of sequence.
+ */
+int qsgw_sigma_begin(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ, double eta);
+int qsgw_sigma_add_poles(qsgw_sigma_plan *plan, const double *Omega, const double *Z, int64_t ldz, int64_t n_pole);
+int qsgw_sigma_finish(qsgw_sigma_plan *plan, double *Sigma);
+
+/*
+ * Same build with HOST buffers (same shapes and meaning as qsgw_sigma_build): the library uploads
+ * B, eps, occ once and Omega/Z in ranges of one s_block of poles, overlapping the upload of the
+ * next range with the kernels of the current one, downloads Sigma and synchronises before returning.
+ * n_pole may exceed n_pole_max.  Device staging buffers for the host path are allocated on the first
+ * call (not in create) and kept by the plan; ALLOC if they do not fit.
+ */
+int qsgw_sigma_build_host(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ,
+                          const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
+                          double *Sigma);
+
+/* Free the workspace and the plan.  Synchronises the plan's stream first.  NULL is accepted. */
+int qsgw_sigma_destroy(qsgw_sigma_plan *plan);
+
+/* ---- helpers, not part of the method ---- */
+
+/* Message for the most recent failure on this plan ("" if none); valid until the next call on the plan.
+ * With plan == NULL: message for the most recent failed qsgw_sigma_create on this thread. */
+const char *qsgw_sigma_last_error(const qsgw_sigma_plan *plan);
+
+/* Device bytes the plan allocated (workspace + host-path staging so far). */
+size_t qsgw_sigma_workspace_bytes(const qsgw_sigma_plan *plan);
+
+/* Profiling on (1) / off (0): when on, every kernel launch is bracketed by CUDA events on the plan's
+ * stream and qsgw_sigma_get_stats sums them per stage.  Off by default. */
+int qsgw_sigma_set_profiling(qsgw_sigma_plan *plan, int on);
+/* Synchronises the stream, fills *stats with the totals since the last reset; reset != 0 clears them. */
+int qsgw_sigma_get_stats(qsgw_sigma_plan *plan, qsgw_sigma_stats *stats, int reset);
+
+/* Test/debug helper: copy the leading rows x cols block of a workspace array into a dense device buffer
+ * dst[rows][cols], asynchronously on the plan's stream.  which: 0 = V of the last chunk [n_aux][s],
+ * 1 = w chunk of the last chunk [n_mo*n_mo][s] (row m*n_mo+p), 2 = packed symmetric B [n_aux][n_mo(n_mo+1)/2],
+ * 3 = transposed ov block [n_occ*n_virt][n_aux], 4 = split-K partial tiles [nsplit][n_mo*n_mo] (rows = nsplit).
+ * INVALID_ARG if the block exceeds the array. */
+int qsgw_sigma_copy_workspace(qsgw_sigma_plan *plan, int which, double *dst, int64_t rows, int64_t cols);
+
+/* Library version (major*10000 + minor*100 + patch). */
+int qsgw_sigma_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QSGW_SIGMA_H */

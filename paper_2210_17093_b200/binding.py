@@ -1,0 +1,244 @@
+"""Thin ctypes binding of include/qsgw_sigma.h: argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libqsgw_sigma.so; PyTorch is used for
+device memory and streams.  There is no CPU fallback: if the shared library is missing or
+there is no CUDA device the calls raise.  Function names are the C names.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqsgw_sigma.so")
+
+QSGW_SIGMA_OK = 0
+QSGW_SIGMA_ERR_INVALID_ARG = -1
+QSGW_SIGMA_ERR_ALLOC = -2
+QSGW_SIGMA_ERR_CUDA = -3
+
+EXPORTS = (
+    "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
+    "qsgw_sigma_build_host", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
+    "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_copy_workspace", "qsgw_sigma_version",
+)
+
+
+class QsgwSigmaError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"qsgw_sigma error {code}: {message}")
+        self.code = code
+
+
+class qsgw_sigma_stats(ctypes.Structure):
+    _fields_ = [
+        ("ms_pack", ctypes.c_double), ("launches_pack", ctypes.c_int64),
+        ("ms_stage1", ctypes.c_double), ("launches_stage1", ctypes.c_int64),
+        ("ms_stage2", ctypes.c_double), ("launches_stage2", ctypes.c_int64),
+        ("ms_stage3", ctypes.c_double), ("launches_stage3", ctypes.c_int64),
+        ("ms_epilogue", ctypes.c_double), ("launches_epilogue", ctypes.c_int64),
+        ("builds", ctypes.c_int64), ("poles", ctypes.c_int64),
+    ]
+
+    def as_dict(self):
+        return {name: getattr(self, name) for name, _ in self._fields_}
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen the in-tree libqsgw_sigma.so (built by paper_2210_17093_b200.build); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} not found: build it with `python -m paper_2210_17093_b200.build` "
+                "(there is no CPU fallback for the qsGW Sigma build)")
+        lib = ctypes.CDLL(LIB_PATH)
+        vp, dp, i64, ci, cd = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
+        lib.qsgw_sigma_create.restype = ci
+        lib.qsgw_sigma_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, i64, ci, vp]
+        lib.qsgw_sigma_build.restype = ci
+        lib.qsgw_sigma_build.argtypes = [vp, dp, dp, dp, dp, dp, i64, i64, cd, dp]
+        lib.qsgw_sigma_begin.restype = ci
+        lib.qsgw_sigma_begin.argtypes = [vp, dp, dp, dp, cd]
+        lib.qsgw_sigma_add_poles.restype = ci
+        lib.qsgw_sigma_add_poles.argtypes = [vp, dp, dp, i64, i64]
+        lib.qsgw_sigma_finish.restype = ci
+        lib.qsgw_sigma_finish.argtypes = [vp, dp]
+        lib.qsgw_sigma_build_host.restype = ci
+        lib.qsgw_sigma_build_host.argtypes = [vp, dp, dp, dp, dp, dp, i64, i64, cd, dp]
+        lib.qsgw_sigma_destroy.restype = ci
+        lib.qsgw_sigma_destroy.argtypes = [vp]
+        lib.qsgw_sigma_last_error.restype = ctypes.c_char_p
+        lib.qsgw_sigma_last_error.argtypes = [vp]
+        lib.qsgw_sigma_workspace_bytes.restype = ctypes.c_size_t
+        lib.qsgw_sigma_workspace_bytes.argtypes = [vp]
+        lib.qsgw_sigma_set_profiling.restype = ci
+        lib.qsgw_sigma_set_profiling.argtypes = [vp, ci]
+        lib.qsgw_sigma_get_stats.restype = ci
+        lib.qsgw_sigma_get_stats.argtypes = [vp, ctypes.POINTER(qsgw_sigma_stats), ci]
+        lib.qsgw_sigma_copy_workspace.restype = ci
+        lib.qsgw_sigma_copy_workspace.argtypes = [vp, ci, dp, i64, i64]
+        lib.qsgw_sigma_version.restype = ci
+        lib.qsgw_sigma_version.argtypes = []
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, plan) -> None:
+    if rc != QSGW_SIGMA_OK:
+        msg = load_library().qsgw_sigma_last_error(plan)
+        raise QsgwSigmaError(rc, msg.decode() if msg else "")
+
+
+def _dev(t: torch.Tensor, name: str, shape=None) -> int:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64:
+        raise TypeError(f"{name} must be a CUDA float64 tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return t.data_ptr()
+
+
+def _host(t: torch.Tensor, name: str, shape=None) -> int:
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError(f"{name} must be a contiguous host float64 tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return t.data_ptr()
+
+
+class Plan:
+    """Handle returned by qsgw_sigma_create (holds the opaque qsgw_sigma_plan* and the sizes)."""
+
+    def __init__(self, handle, n_mo, n_occ, n_aux, n_pole_max, s_block, stream):
+        self.handle, self.n_mo, self.n_occ, self.n_aux = handle, n_mo, n_occ, n_aux
+        self.n_pole_max, self.s_block, self.stream = n_pole_max, s_block, stream
+        self.n_ov = n_occ * (n_mo - n_occ)
+
+    def __del__(self):
+        try:
+            qsgw_sigma_destroy(self)
+        except Exception:
+            pass
+
+
+def qsgw_sigma_create(n_mo: int, n_occ: int, n_aux: int, n_pole_max: int, s_block: int = 0,
+                      stream: Optional[torch.cuda.Stream] = None) -> Plan:
+    lib = load_library()
+    if stream is None and torch.cuda.is_available():
+        stream = torch.cuda.current_stream()
+    sptr = ctypes.c_void_p(stream.cuda_stream if stream is not None else 0)
+    h = ctypes.c_void_p()
+    rc = lib.qsgw_sigma_create(ctypes.byref(h), int(n_mo), int(n_occ), int(n_aux), int(n_pole_max), int(s_block), sptr)
+    _check(rc, None)
+    return Plan(h, n_mo, n_occ, n_aux, n_pole_max, s_block, stream)
+
+
+def _z_args(plan: Plan, Omega: torch.Tensor, Z: torch.Tensor, ptr):
+    n_pole = Omega.shape[0]
+    if Z.dim() != 2 or Z.shape != (plan.n_ov, n_pole) or Z.stride(1) != 1:
+        raise ValueError(f"Z must be [{plan.n_ov}, {n_pole}] with unit column stride (a column slice of a larger Z is fine)")
+    if not Omega.is_contiguous():
+        raise ValueError("Omega must be contiguous")
+    return ptr(Omega, "Omega"), ptr(Z, "Z"), int(Z.stride(0)) if Z.shape[0] > 1 else max(n_pole, int(Z.stride(0))), n_pole
+
+
+def qsgw_sigma_build(plan: Plan, B, eps, occ, Omega, Z, eta: float, Sigma: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Sigma (Eq. 19) for the poles handed in; asynchronous on the plan's stream.  Z may be a column slice."""
+    N = plan.n_mo
+    if not B.is_contiguous() or not eps.is_contiguous() or not occ.is_contiguous():
+        raise ValueError("B, eps, occ must be contiguous")
+    if Sigma is None:
+        Sigma = torch.empty((N, N), dtype=torch.float64, device=B.device)
+    om, z, ldz, n_pole = _z_args(plan, Omega, Z, _dev)
+    rc = load_library().qsgw_sigma_build(plan.handle, _dev(B, "B", (plan.n_aux, N, N)), _dev(eps, "eps", (N,)),
+                                         _dev(occ, "occ", (N,)), om, z, ldz, n_pole, float(eta),
+                                         _dev(Sigma, "Sigma", (N, N)))
+    _check(rc, plan.handle)
+    return Sigma
+
+
+def qsgw_sigma_begin(plan: Plan, B, eps, occ, eta: float) -> None:
+    N = plan.n_mo
+    if not B.is_contiguous() or not eps.is_contiguous() or not occ.is_contiguous():
+        raise ValueError("B, eps, occ must be contiguous")
+    rc = load_library().qsgw_sigma_begin(plan.handle, _dev(B, "B", (plan.n_aux, N, N)), _dev(eps, "eps", (N,)),
+                                         _dev(occ, "occ", (N,)), float(eta))
+    _check(rc, plan.handle)
+
+
+def qsgw_sigma_add_poles(plan: Plan, Omega, Z) -> None:
+    om, z, ldz, n_pole = _z_args(plan, Omega, Z, _dev)
+    _check(load_library().qsgw_sigma_add_poles(plan.handle, om, z, ldz, n_pole), plan.handle)
+
+
+def qsgw_sigma_finish(plan: Plan, Sigma: Optional[torch.Tensor] = None) -> torch.Tensor:
+    N = plan.n_mo
+    if Sigma is None:
+        Sigma = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    _check(load_library().qsgw_sigma_finish(plan.handle, _dev(Sigma, "Sigma", (N, N))), plan.handle)
+    return Sigma
+
+
+def qsgw_sigma_build_host(plan: Plan, B, eps, occ, Omega, Z, eta: float, Sigma: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Same build from HOST tensors (pinned or pageable); uploads, builds, downloads, synchronises."""
+    N = plan.n_mo
+    if Sigma is None:
+        Sigma = torch.empty((N, N), dtype=torch.float64)
+    om, z, ldz, n_pole = _z_args(plan, Omega, Z, _host_strided)
+    rc = load_library().qsgw_sigma_build_host(plan.handle, _host(B, "B", (plan.n_aux, N, N)), _host(eps, "eps", (N,)),
+                                              _host(occ, "occ", (N,)), om, z, ldz, n_pole, float(eta),
+                                              _host(Sigma, "Sigma", (N, N)))
+    _check(rc, plan.handle)
+    return Sigma
+
+
+def _host_strided(t: torch.Tensor, name: str) -> int:
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.float64:
+        raise TypeError(f"{name} must be a host float64 tensor")
+    return t.data_ptr()
+
+
+def qsgw_sigma_destroy(plan: Plan) -> None:
+    if plan is not None and plan.handle is not None and plan.handle.value:
+        h, plan.handle = plan.handle, ctypes.c_void_p()
+        load_library().qsgw_sigma_destroy(h)
+
+
+def qsgw_sigma_last_error(plan: Optional[Plan]) -> str:
+    msg = load_library().qsgw_sigma_last_error(plan.handle if plan is not None else None)
+    return msg.decode() if msg else ""
+
+
+def qsgw_sigma_workspace_bytes(plan: Plan) -> int:
+    return int(load_library().qsgw_sigma_workspace_bytes(plan.handle))
+
+
+def qsgw_sigma_set_profiling(plan: Plan, on: bool) -> None:
+    _check(load_library().qsgw_sigma_set_profiling(plan.handle, 1 if on else 0), plan.handle)
+
+
+def qsgw_sigma_get_stats(plan: Plan, reset: bool = False) -> dict:
+    st = qsgw_sigma_stats()
+    _check(load_library().qsgw_sigma_get_stats(plan.handle, ctypes.byref(st), 1 if reset else 0), plan.handle)
+    return st.as_dict()
+
+
+WORKSPACE_V, WORKSPACE_W, WORKSPACE_BP, WORKSPACE_BOVT, WORKSPACE_TPART = range(5)
+
+
+def qsgw_sigma_copy_workspace(plan: Plan, which: int, rows: int, cols: int) -> torch.Tensor:
+    """Test/debug helper: dense copy of the leading rows x cols block of a workspace array."""
+    out = torch.empty((rows, cols), dtype=torch.float64, device="cuda")
+    _check(load_library().qsgw_sigma_copy_workspace(plan.handle, int(which), out.data_ptr(), int(rows), int(cols)),
+           plan.handle)
+    return out
+
+
+def qsgw_sigma_version() -> int:
+    return int(load_library().qsgw_sigma_version())

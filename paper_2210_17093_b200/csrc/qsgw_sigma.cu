@@ -1,0 +1,480 @@
+// qsgw_sigma.cu -- plan, workspace, stage scheduler and the C ABI of include/qsgw_sigma.h.
+//
+// Path per pole chunk (<= s_block poles):  stage 1 GEMM (V) -> stage 2 GEMM (w chunk, symmetric pairs,
+// scattered to both mirrors) -> stage 3 fused D-scaling + contraction into split-K partial tiles.
+// begin() packs B once per Sigma; finish() reduces the partial tiles in fixed order and symmetrises.
+// Everything is enqueued on the plan's stream; no call allocates except create (and the first host-path call).
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/qsgw_sigma.h"
+#include "sigma_kernels.cuh"
+
+using namespace qsgw;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+enum StageId { kPack = 0, kStage1, kStage2, kStage3, kEpilogue, kNumStages };
+
+struct EventPair {
+  cudaEvent_t a, b;
+};
+
+}  // namespace
+
+struct qsgw_sigma_plan {
+  int n_mo = 0, n_occ = 0, n_virt = 0, n_aux = 0;
+  int64_t n_ov = 0, n_pole_max = 0;
+  int s_chunk = 0;
+  cudaStream_t stream = nullptr;
+  int device = 0;
+
+  // workspace
+  int64_t n_pair = 0, ldp = 0, ld_aux = 0, ldv = 0, ldw = 0;
+  int nsplit = 0, m_per_split = 0, ntile_1d = 0;
+  double *Bp = nullptr, *BovT = nullptr, *V = nullptr, *W = nullptr, *Tpart = nullptr;
+  int2 *pairs = nullptr;
+  size_t bytes = 0;
+
+  // state of the current Sigma
+  bool begun = false;
+  const double *B = nullptr, *eps = nullptr, *occ = nullptr;
+  double eta = 0.0;
+
+  // host path staging (allocated lazily)
+  double *hB = nullptr, *hEps = nullptr, *hOcc = nullptr, *hSigma = nullptr;
+  double *hOmega[2] = {nullptr, nullptr}, *hZ[2] = {nullptr, nullptr};
+  int64_t h_range = 0;
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr};
+
+  // profiling
+  bool profiling = false;
+  std::vector<EventPair> pending[kNumStages];
+  std::vector<EventPair> pool;
+  double ms[kNumStages] = {0, 0, 0, 0, 0};
+  int64_t launches[kNumStages] = {0, 0, 0, 0, 0};
+  int64_t builds = 0, poles = 0;
+
+  std::string err;
+};
+
+namespace {
+
+int fail(qsgw_sigma_plan *p, int code, const std::string &msg) {
+  if (p) p->err = msg; else g_create_error = msg;
+  return code;
+}
+
+#define QSGW_CUDA(plan, expr)                                                                              \
+  do {                                                                                                     \
+    cudaError_t e_ = (expr);                                                                               \
+    if (e_ != cudaSuccess)                                                                                 \
+      return fail((plan), QSGW_SIGMA_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));        \
+  } while (0)
+
+template <class T>
+int dev_alloc(qsgw_sigma_plan *p, T **ptr, size_t count, const char *what) {
+  void *q = nullptr;
+  const size_t nbytes = std::max<size_t>(count, 1) * sizeof(T);
+  cudaError_t e = cudaMalloc(&q, nbytes);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    char buf[256];
+    snprintf(buf, sizeof buf, "cudaMalloc of %.3f GB for %s failed: %s", nbytes / 1e9, what, cudaGetErrorString(e));
+    return fail(p, QSGW_SIGMA_ERR_ALLOC, buf);
+  }
+  *ptr = static_cast<T *>(q);
+  p->bytes += nbytes;
+  return QSGW_SIGMA_OK;
+}
+
+inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+struct ScopedTimer {  // brackets one launch with events when profiling is on
+  qsgw_sigma_plan *p;
+  StageId id;
+  EventPair ev{nullptr, nullptr};
+  ScopedTimer(qsgw_sigma_plan *plan, StageId stage) : p(plan), id(stage) {
+    if (!p->profiling) return;
+    if (!p->pool.empty()) {
+      ev = p->pool.back();
+      p->pool.pop_back();
+    } else {
+      cudaEventCreate(&ev.a);
+      cudaEventCreate(&ev.b);
+    }
+    cudaEventRecord(ev.a, p->stream);
+  }
+  ~ScopedTimer() {
+    if (!p->profiling) return;
+    cudaEventRecord(ev.b, p->stream);
+    p->pending[id].push_back(ev);
+  }
+};
+
+void drain_events(qsgw_sigma_plan *p) {
+  for (int s = 0; s < kNumStages; ++s) {
+    for (EventPair &ev : p->pending[s]) {
+      float t = 0.f;
+      if (cudaEventElapsedTime(&t, ev.a, ev.b) == cudaSuccess) {
+        p->ms[s] += t;
+        p->launches[s] += 1;
+      }
+      p->pool.push_back(ev);
+    }
+    p->pending[s].clear();
+  }
+}
+
+template <int VECB, class Epi>
+int launch_gemm(qsgw_sigma_plan *p, const double *A, int64_t lda, const double *Bm, int64_t ldb, int M, int N, int K,
+                const Epi &epi) {
+  static bool configured = false;
+  auto kern = gemm_tn_dmma_kernel<VECB, Epi>;
+  if (!configured) {
+    QSGW_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGemmSmemBytes));
+    configured = true;
+  }
+  const int ntm = (M + kBM - 1) / kBM, ntn = (N + kBN - 1) / kBN;
+  kern<<<ntm * ntn, kThreads, kGemmSmemBytes, p->stream>>>(A, lda, Bm, ldb, M, N, K, ntn, epi);
+  QSGW_CUDA(p, cudaGetLastError());
+  return QSGW_SIGMA_OK;
+}
+
+inline bool aligned16(const void *ptr, int64_t ld) { return (reinterpret_cast<uintptr_t>(ptr) & 15) == 0 && (ld & 1) == 0; }
+
+int check_plan(qsgw_sigma_plan *p) {
+  if (!p) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "plan is NULL");
+  cudaError_t e = cudaSetDevice(p->device);
+  if (e != cudaSuccess) return fail(p, QSGW_SIGMA_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
+  return QSGW_SIGMA_OK;
+}
+
+int do_begin(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, double eta) {
+  if (!B || !eps || !occ) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "begin: B, eps and occ must be non-NULL");
+  if (!(eta > 0.0) || !std::isfinite(eta)) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "begin: eta must be finite and > 0");
+  p->B = B; p->eps = eps; p->occ = occ; p->eta = eta;
+  {
+    ScopedTimer t(p, kPack);
+    pack_pairs_kernel<<<dim3(p->n_mo, p->n_aux), 128, 0, p->stream>>>(B, p->n_mo, p->Bp, p->ldp);
+    QSGW_CUDA(p, cudaGetLastError());
+    dim3 grid((p->n_virt + 31) / 32, (p->n_aux + 31) / 32, p->n_occ);
+    pack_ov_transposed_kernel<<<grid, dim3(32, 8), 0, p->stream>>>(B, p->n_mo, p->n_occ, p->n_aux, p->BovT, p->ld_aux);
+    QSGW_CUDA(p, cudaGetLastError());
+  }
+  QSGW_CUDA(p, cudaMemsetAsync(p->Tpart, 0, sizeof(double) * (size_t)p->nsplit * p->n_mo * p->n_mo, p->stream));
+  p->begun = true;
+  return QSGW_SIGMA_OK;
+}
+
+int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64_t ldz, int64_t n_pole) {
+  if (!p->begun) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles called before begin");
+  if (!Omega || !Z) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles: Omega and Z must be non-NULL");
+  if (n_pole < 1 || n_pole > p->n_pole_max)
+    return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles: n_pole must be in [1, n_pole_max]");
+  if (ldz < n_pole) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles: ldz < n_pole");
+
+  static bool sigma_configured = false;
+  if (!sigma_configured) {
+    QSGW_CUDA(p, cudaFuncSetAttribute(sigma_accumulate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)kSigmaSmemBytes));
+    sigma_configured = true;
+  }
+  const int nt = (p->n_mo + kBM - 1) / kBM;
+  for (int64_t c0 = 0; c0 < n_pole; c0 += p->s_chunk) {
+    const int sc = (int)std::min<int64_t>(p->s_chunk, n_pole - c0);
+    const double *Zc = Z + c0;
+    {  // stage 1: V[P][s] = sum_ia BovT[ia][P] * Z[ia][c0+s]
+      ScopedTimer t(p, kStage1);
+      EpiStore epi{p->V, p->ldv, 1.0};
+      int rc = aligned16(Zc, ldz)
+                   ? launch_gemm<2>(p, p->BovT, p->ld_aux, Zc, ldz, p->n_aux, sc, (int)p->n_ov, epi)
+                   : launch_gemm<1>(p, p->BovT, p->ld_aux, Zc, ldz, p->n_aux, sc, (int)p->n_ov, epi);
+      if (rc) return rc;
+    }
+    {  // stage 2: w[(p<=m)][s] = sqrt(2) sum_P Bp[P][(p,m)] * V[P][s], scattered to W[(m,p)] and W[(p,m)]
+      ScopedTimer t(p, kStage2);
+      EpiPairScatter epi{p->W, p->ldw, p->pairs, p->n_mo, std::sqrt(2.0)};
+      int rc = launch_gemm<2>(p, p->Bp, p->ldp, p->V, p->ldv, (int)p->n_pair, sc, p->n_aux, epi);
+      if (rc) return rc;
+    }
+    {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
+      ScopedTimer t(p, kStage3);
+      sigma_accumulate_kernel<<<dim3(nt * nt, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
+          p->W, p->ldw, p->eps, p->occ, Omega + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, nt, p->Tpart);
+      QSGW_CUDA(p, cudaGetLastError());
+    }
+  }
+  p->poles += n_pole;
+  return QSGW_SIGMA_OK;
+}
+
+int do_finish(qsgw_sigma_plan *p, double *Sigma) {
+  if (!p->begun) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "finish called before begin");
+  if (!Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "finish: Sigma must be non-NULL");
+  {
+    ScopedTimer t(p, kEpilogue);
+    const int nb = (p->n_mo + 31) / 32;
+    sigma_epilogue_kernel<<<dim3(nb, nb), dim3(32, 8), 0, p->stream>>>(p->Tpart, p->nsplit, p->n_mo, Sigma);
+    QSGW_CUDA(p, cudaGetLastError());
+  }
+  p->begun = false;
+  p->builds += 1;
+  return QSGW_SIGMA_OK;
+}
+
+int ensure_host_staging(qsgw_sigma_plan *p) {
+  if (p->hB) return QSGW_SIGMA_OK;
+  const int64_t range = p->s_chunk;   // one w chunk per uploaded pole range
+  const size_t nn = (size_t)p->n_mo * p->n_mo;
+  int rc;
+  if ((rc = dev_alloc(p, &p->hB, (size_t)p->n_aux * nn, "host-path B"))) return rc;
+  if ((rc = dev_alloc(p, &p->hEps, p->n_mo, "host-path eps"))) return rc;
+  if ((rc = dev_alloc(p, &p->hOcc, p->n_mo, "host-path occ"))) return rc;
+  if ((rc = dev_alloc(p, &p->hSigma, nn, "host-path Sigma"))) return rc;
+  const int64_t ld = round_up(range, 2);
+  for (int b = 0; b < 2; ++b) {
+    if ((rc = dev_alloc(p, &p->hOmega[b], ld, "host-path Omega"))) return rc;
+    if ((rc = dev_alloc(p, &p->hZ[b], (size_t)p->n_ov * ld, "host-path Z range"))) return rc;
+    QSGW_CUDA(p, cudaEventCreateWithFlags(&p->ev_copied[b], cudaEventDisableTiming));
+    QSGW_CUDA(p, cudaEventCreateWithFlags(&p->ev_consumed[b], cudaEventDisableTiming));
+  }
+  QSGW_CUDA(p, cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+  p->h_range = range;
+  return QSGW_SIGMA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int qsgw_sigma_version(void) { return 100; }
+
+int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, int64_t n_pole_max, int s_block,
+                      void *cuda_stream) {
+  if (!plan) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "create: plan is NULL");
+  *plan = nullptr;
+  if (n_mo < 2 || n_occ < 1 || n_occ >= n_mo || n_aux < 1 || n_pole_max < 1 || s_block < 0)
+    return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG,
+                "create: need n_mo >= 2, 1 <= n_occ < n_mo, n_aux >= 1, n_pole_max >= 1, s_block >= 0");
+  if ((int64_t)n_occ * (n_mo - n_occ) > INT32_MAX || (int64_t)n_mo * (n_mo + 1) / 2 > INT32_MAX)
+    return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "create: n_mo too large for 32-bit tile indices");
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, QSGW_SIGMA_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
+  }
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, QSGW_SIGMA_ERR_CUDA, std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e));
+  }
+  if (prop.major != 10)
+    return fail(nullptr, QSGW_SIGMA_ERR_CUDA, "this library is built for sm_100a (B200) only; device is " +
+                                                  std::string(prop.name));
+
+  qsgw_sigma_plan *p = new (std::nothrow) qsgw_sigma_plan;
+  if (!p) return fail(nullptr, QSGW_SIGMA_ERR_ALLOC, "create: out of host memory");
+  p->device = dev;
+  p->n_mo = n_mo; p->n_occ = n_occ; p->n_virt = n_mo - n_occ; p->n_aux = n_aux;
+  p->n_ov = (int64_t)n_occ * p->n_virt;
+  p->n_pole_max = n_pole_max;
+  p->stream = static_cast<cudaStream_t>(cuda_stream);
+  int64_t chunk = s_block > 0 ? s_block : 2048;
+  chunk = std::min<int64_t>(chunk, n_pole_max);
+  p->s_chunk = (int)round_up(chunk, 2);          // even chunk starts keep Z + c0 16-byte aligned when ldz is even
+  p->n_pair = (int64_t)n_mo * (n_mo + 1) / 2;
+  p->ldp = round_up(p->n_pair, 2);
+  p->ld_aux = round_up(n_aux, 2);
+  p->ldv = round_up(p->s_chunk, 2);
+  p->ldw = round_up(p->s_chunk, 2);
+  // split-K of stage 3 over the internal state m: enough CTAs for >= ~16 waves of the SMs, at most N splits
+  const int nt = (n_mo + kBM - 1) / kBM;
+  int want = (16 * prop.multiProcessorCount + nt * nt - 1) / (nt * nt);
+  want = std::max(1, std::min(want, n_mo));
+  p->m_per_split = (n_mo + want - 1) / want;
+  p->nsplit = (n_mo + p->m_per_split - 1) / p->m_per_split;
+
+  int rc;
+  auto bail = [&](int code) {
+    std::string msg = p->err;
+    qsgw_sigma_destroy(p);
+    return fail(nullptr, code, msg);
+  };
+  if ((rc = dev_alloc(p, &p->Bp, (size_t)n_aux * p->ldp, "packed symmetric B"))) return bail(rc);
+  if ((rc = dev_alloc(p, &p->BovT, (size_t)p->n_ov * p->ld_aux, "transposed ov block of B"))) return bail(rc);
+  if ((rc = dev_alloc(p, &p->V, (size_t)n_aux * p->ldv, "V chunk"))) return bail(rc);
+  if ((rc = dev_alloc(p, &p->W, (size_t)n_mo * n_mo * p->ldw, "w chunk"))) return bail(rc);
+  if ((rc = dev_alloc(p, &p->Tpart, (size_t)p->nsplit * n_mo * n_mo, "split-K partial tiles"))) return bail(rc);
+  if ((rc = dev_alloc(p, &p->pairs, (size_t)p->ldp, "pair table"))) return bail(rc);
+  pair_table_kernel<<<n_mo, 128, 0, p->stream>>>(n_mo, p->pairs);
+  e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+  if (e != cudaSuccess) {
+    p->err = std::string("pair table kernel: ") + cudaGetErrorString(e);
+    return bail(QSGW_SIGMA_ERR_CUDA);
+  }
+  *plan = p;
+  return QSGW_SIGMA_OK;
+}
+
+int qsgw_sigma_begin(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, double eta) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  return do_begin(p, B, eps, occ, eta);
+}
+
+int qsgw_sigma_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64_t ldz, int64_t n_pole) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  return do_add_poles(p, Omega, Z, ldz, n_pole);
+}
+
+int qsgw_sigma_finish(qsgw_sigma_plan *p, double *Sigma) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  return do_finish(p, Sigma);
+}
+
+int qsgw_sigma_build(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, const double *Omega,
+                     const double *Z, int64_t ldz, int64_t n_pole, double eta, double *Sigma) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  if (!Omega || !Z || !Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build: NULL argument");
+  if (n_pole < 1 || n_pole > p->n_pole_max) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build: n_pole must be in [1, n_pole_max]");
+  if (ldz < n_pole) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build: ldz < n_pole");
+  if ((rc = do_begin(p, B, eps, occ, eta))) return rc;
+  if ((rc = do_add_poles(p, Omega, Z, ldz, n_pole))) { p->begun = false; return rc; }
+  return do_finish(p, Sigma);
+}
+
+int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ,
+                          const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
+                          double *Sigma) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  if (!B || !eps || !occ || !Omega || !Z || !Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build_host: NULL argument");
+  if (n_pole < 1 || ldz < n_pole) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build_host: need 1 <= n_pole <= ldz");
+  if (!(eta > 0.0)) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build_host: eta must be > 0");
+  if ((rc = ensure_host_staging(p))) return rc;
+  const int64_t R = p->h_range, ldr = round_up(R, 2);
+  const size_t nn = (size_t)p->n_mo * p->n_mo;
+
+  // B, eps, occ on the compute stream (begin needs them first)
+  QSGW_CUDA(p, cudaMemcpyAsync(p->hB, B, sizeof(double) * p->n_aux * nn, cudaMemcpyHostToDevice, p->stream));
+  QSGW_CUDA(p, cudaMemcpyAsync(p->hEps, eps, sizeof(double) * p->n_mo, cudaMemcpyHostToDevice, p->stream));
+  QSGW_CUDA(p, cudaMemcpyAsync(p->hOcc, occ, sizeof(double) * p->n_mo, cudaMemcpyHostToDevice, p->stream));
+
+  // pole ranges: upload range r+1 on the copy stream while the compute stream works on range r
+  auto upload = [&](int64_t s0, int buf) -> int {
+    const int64_t n = std::min<int64_t>(R, n_pole - s0);
+    QSGW_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->ev_consumed[buf], 0));
+    QSGW_CUDA(p, cudaMemcpyAsync(p->hOmega[buf], Omega + s0, sizeof(double) * n, cudaMemcpyHostToDevice, p->copy_stream));
+    QSGW_CUDA(p, cudaMemcpy2DAsync(p->hZ[buf], sizeof(double) * ldr, Z + s0, sizeof(double) * ldz, sizeof(double) * n,
+                                   (size_t)p->n_ov, cudaMemcpyHostToDevice, p->copy_stream));
+    QSGW_CUDA(p, cudaEventRecord(p->ev_copied[buf], p->copy_stream));
+    return QSGW_SIGMA_OK;
+  };
+  // both buffers start out free
+  QSGW_CUDA(p, cudaEventRecord(p->ev_consumed[0], p->stream));
+  QSGW_CUDA(p, cudaEventRecord(p->ev_consumed[1], p->stream));
+  if ((rc = upload(0, 0))) return rc;
+  if ((rc = do_begin(p, p->hB, p->hEps, p->hOcc, eta))) return rc;
+  int buf = 0;
+  for (int64_t s0 = 0; s0 < n_pole; s0 += R, buf ^= 1) {
+    const int64_t n = std::min<int64_t>(R, n_pole - s0);
+    if (s0 + R < n_pole && (rc = upload(s0 + R, buf ^ 1))) { p->begun = false; return rc; }
+    QSGW_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_copied[buf], 0));
+    if ((rc = do_add_poles(p, p->hOmega[buf], p->hZ[buf], ldr, n))) { p->begun = false; return rc; }
+    QSGW_CUDA(p, cudaEventRecord(p->ev_consumed[buf], p->stream));
+  }
+  if ((rc = do_finish(p, p->hSigma))) return rc;
+  QSGW_CUDA(p, cudaMemcpyAsync(Sigma, p->hSigma, sizeof(double) * nn, cudaMemcpyDeviceToHost, p->stream));
+  QSGW_CUDA(p, cudaStreamSynchronize(p->stream));
+  return QSGW_SIGMA_OK;
+}
+
+int qsgw_sigma_destroy(qsgw_sigma_plan *p) {
+  if (!p) return QSGW_SIGMA_OK;
+  cudaSetDevice(p->device);
+  cudaStreamSynchronize(p->stream);
+  if (p->copy_stream) { cudaStreamSynchronize(p->copy_stream); cudaStreamDestroy(p->copy_stream); }
+  for (int s = 0; s < kNumStages; ++s)
+    for (EventPair &ev : p->pending[s]) p->pool.push_back(ev);
+  for (EventPair &ev : p->pool) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+  for (int b = 0; b < 2; ++b) {
+    if (p->ev_copied[b]) cudaEventDestroy(p->ev_copied[b]);
+    if (p->ev_consumed[b]) cudaEventDestroy(p->ev_consumed[b]);
+    cudaFree(p->hOmega[b]); cudaFree(p->hZ[b]);
+  }
+  cudaFree(p->hB); cudaFree(p->hEps); cudaFree(p->hOcc); cudaFree(p->hSigma);
+  cudaFree(p->Bp); cudaFree(p->BovT); cudaFree(p->V); cudaFree(p->W); cudaFree(p->Tpart); cudaFree(p->pairs);
+  cudaGetLastError();
+  delete p;
+  return QSGW_SIGMA_OK;
+}
+
+const char *qsgw_sigma_last_error(const qsgw_sigma_plan *p) { return p ? p->err.c_str() : g_create_error.c_str(); }
+
+size_t qsgw_sigma_workspace_bytes(const qsgw_sigma_plan *p) { return p ? p->bytes : 0; }
+
+int qsgw_sigma_set_profiling(qsgw_sigma_plan *p, int on) {
+  if (!p) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "plan is NULL");
+  p->profiling = on != 0;
+  return QSGW_SIGMA_OK;
+}
+
+int qsgw_sigma_copy_workspace(qsgw_sigma_plan *p, int which, double *dst, int64_t rows, int64_t cols) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  if (!dst || rows < 1 || cols < 1) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "copy_workspace: bad arguments");
+  const double *src = nullptr;
+  int64_t ld = 0, max_rows = 0;
+  const int64_t nn = (int64_t)p->n_mo * p->n_mo;
+  switch (which) {
+    case 0: src = p->V; ld = p->ldv; max_rows = p->n_aux; break;
+    case 1: src = p->W; ld = p->ldw; max_rows = nn; break;
+    case 2: src = p->Bp; ld = p->ldp; max_rows = p->n_aux; break;
+    case 3: src = p->BovT; ld = p->ld_aux; max_rows = p->n_ov; break;
+    case 4: src = p->Tpart; ld = nn; max_rows = p->nsplit; break;
+    default: return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "copy_workspace: unknown array");
+  }
+  if (rows > max_rows || cols > ld) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "copy_workspace: block exceeds the array");
+  QSGW_CUDA(p, cudaMemcpy2DAsync(dst, sizeof(double) * cols, src, sizeof(double) * ld, sizeof(double) * cols, (size_t)rows,
+                                 cudaMemcpyDeviceToDevice, p->stream));
+  return QSGW_SIGMA_OK;
+}
+
+int qsgw_sigma_get_stats(qsgw_sigma_plan *p, qsgw_sigma_stats *st, int reset) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  if (!st) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "get_stats: stats is NULL");
+  QSGW_CUDA(p, cudaStreamSynchronize(p->stream));
+  drain_events(p);
+  st->ms_pack = p->ms[kPack];         st->launches_pack = p->launches[kPack];
+  st->ms_stage1 = p->ms[kStage1];     st->launches_stage1 = p->launches[kStage1];
+  st->ms_stage2 = p->ms[kStage2];     st->launches_stage2 = p->launches[kStage2];
+  st->ms_stage3 = p->ms[kStage3];     st->launches_stage3 = p->launches[kStage3];
+  st->ms_epilogue = p->ms[kEpilogue]; st->launches_epilogue = p->launches[kEpilogue];
+  st->builds = p->builds;
+  st->poles = p->poles;
+  if (reset) {
+    for (int s = 0; s < kNumStages; ++s) { p->ms[s] = 0; p->launches[s] = 0; }
+    p->builds = 0; p->poles = 0;
+  }
+  return QSGW_SIGMA_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,68 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads and exports every symbol that
+include/qsgw_sigma.h declares; argument validation that happens before any device work; and the
+product never routes through the oracle."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "qsgw_sigma.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(qsgw_sigma_[a-z_]+)\s*\(", text)))
+
+
+def test_library_builds_and_exports_every_declared_symbol():
+    from paper_2210_17093_b200 import build, binding
+    path = build.build_library()
+    lib = ctypes.CDLL(path)
+    declared = _declared_symbols()
+    assert "qsgw_sigma_create" in declared and "qsgw_sigma_build" in declared and "qsgw_sigma_destroy" in declared
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in include/qsgw_sigma.h but not exported"
+    assert sorted(binding.EXPORTS) == declared          # the Python binding carries the same names
+    import paper_2210_17093_b200 as pkg
+    for name in declared:
+        assert callable(getattr(pkg, name))
+    assert pkg.qsgw_sigma_version() >= 100
+
+
+def test_create_rejects_bad_sizes_before_touching_the_device():
+    import paper_2210_17093_b200 as pkg
+    lib = pkg.load_library()
+    h = ctypes.c_void_p()
+    bad = [(1, 1, 4, 4, 0), (8, 0, 4, 4, 0), (8, 8, 4, 4, 0), (8, 2, 0, 4, 0), (8, 2, 4, 0, 0), (8, 2, 4, 4, -1)]
+    for n_mo, n_occ, n_aux, n_pole, s_block in bad:
+        rc = lib.qsgw_sigma_create(ctypes.byref(h), n_mo, n_occ, n_aux, n_pole, s_block, None)
+        assert rc == pkg.QSGW_SIGMA_ERR_INVALID_ARG and not h.value
+        assert b"create" in lib.qsgw_sigma_last_error(None)
+    assert lib.qsgw_sigma_create(None, 8, 2, 4, 4, 0, None) == pkg.QSGW_SIGMA_ERR_INVALID_ARG
+    assert lib.qsgw_sigma_destroy(None) == pkg.QSGW_SIGMA_OK
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+    import paper_2210_17093_b200 as pkg
+    if torch.cuda.is_available():
+        pytest.skip("this check is for the GPU-less container")
+    with pytest.raises(pkg.QsgwSigmaError) as ei:
+        pkg.qsgw_sigma_create(24, 5, 80, 95)
+    assert ei.value.code == pkg.QSGW_SIGMA_ERR_CUDA
+
+
+def test_product_does_not_import_or_link_the_oracle():
+    pkg_dir = os.path.join(ROOT, "paper_2210_17093_b200")
+    for dirpath, _, files in os.walk(pkg_dir):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in text.lower(), f"{f} mentions the oracle"
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2210_17093_b200" not in text and "from paper_2210_17093_b200" not in text
+            assert "csrc" not in text or f.endswith(".c")   # the C file only names csrc/ in its header comment

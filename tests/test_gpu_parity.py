@@ -1,0 +1,203 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Bar (BASELINE.json north_star): max|Sigma_gpu - Sigma_ref| <= 1e-9 * max|Sigma_ref|."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import qsgw_inputs as qi
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-9
+
+
+def _pkg():
+    import paper_2210_17093_b200 as pkg
+    return pkg
+
+
+def _to_dev(inp):
+    return [t.cuda() for t in (inp.B, inp.eps, inp.occ, inp.Omega, inp.Z)]
+
+
+def _gpu_sigma(cfg, dev, s_block=None, n_pole_max=None):
+    pkg = _pkg()
+    B, eps, occ, Om, Z = dev
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, n_pole_max or Om.shape[0],
+                                 cfg.s_block if s_block is None else s_block)
+    S = pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta)
+    torch.cuda.synchronize()
+    return S, plan
+
+
+def _ref_sigma(cfg, inp, states=None):
+    return oracle.sigma(inp.B.numpy(), inp.eps.numpy(), inp.occ.numpy(), inp.Omega.numpy(), inp.Z.numpy(),
+                        cfg.eta, cfg.n_occ, states=states)
+
+
+def _assert_parity(S_gpu, S_ref, tol=TOL):
+    S_gpu = S_gpu.cpu().numpy() if isinstance(S_gpu, torch.Tensor) else S_gpu
+    err = np.max(np.abs(S_gpu - S_ref))
+    scale = np.max(np.abs(S_ref))
+    assert np.all(np.isfinite(S_gpu))
+    assert err <= tol * scale, f"max|dSigma| = {err:.3e} > {tol:g} * max|Sigma_ref| = {tol * scale:.3e}"
+
+
+@pytest.mark.parametrize("name", ["tiny", "small"])
+def test_config_full_parity(name):
+    cfg = qi.CONFIGS[name]
+    inp = qi.make_inputs(cfg)
+    S, plan = _gpu_sigma(cfg, _to_dev(inp))
+    _assert_parity(S, _ref_sigma(cfg, inp))
+    assert torch.equal(S, S.T), "Sigma must be bit-symmetric"
+    _pkg().qsgw_sigma_destroy(plan)
+
+
+# ragged shapes: odd N (scalar epilogues), odd naux, pole counts that leave ragged k / n tails, several
+# chunks with a short last chunk, N spanning 2-3 tiles with a ragged last tile
+RAGGED = [
+    # n_mo n_occ n_aux n_pole s_block
+    (37, 7, 53, 210, 64),
+    (130, 3, 17, 381, 128),
+    (131, 64, 33, 150, 0),
+    (257, 5, 40, 300, 100),
+    (24, 23, 9, 23, 0),
+    (2, 1, 1, 1, 0),
+]
+
+
+@pytest.mark.parametrize("n_mo,n_occ,n_aux,n_pole,s_block", RAGGED)
+def test_ragged_shapes_parity(n_mo, n_occ, n_aux, n_pole, s_block):
+    cfg = qi.custom_config(n_mo, n_occ, n_aux, n_pole=n_pole, s_block=s_block, seed=100 + n_mo)
+    inp = qi.make_inputs(cfg)
+    S, plan = _gpu_sigma(cfg, _to_dev(inp))
+    _assert_parity(S, _ref_sigma(cfg, inp))
+    assert torch.equal(S, S.T)
+    _pkg().qsgw_sigma_destroy(plan)
+
+
+def test_stage_outputs_match_oracle_steps():
+    """a1/a2: V and the w chunk, element by element, against oracle steps 1 and 2."""
+    pkg = _pkg()
+    cfg = qi.custom_config(70, 9, 45, n_pole=200, s_block=0, seed=5)
+    inp = qi.make_inputs(cfg)
+    S, plan = _gpu_sigma(cfg, _to_dev(inp))
+    V = pkg.qsgw_sigma_copy_workspace(plan, pkg.WORKSPACE_V, cfg.n_aux, cfg.n_pole).cpu().numpy()
+    W = pkg.qsgw_sigma_copy_workspace(plan, pkg.WORKSPACE_W, cfg.n_mo ** 2, cfg.n_pole).cpu().numpy()
+    torch.cuda.synchronize()
+    V_ref = oracle.pole_weights(inp.B.numpy(), inp.Z.numpy(), cfg.n_occ)
+    assert np.max(np.abs(V - V_ref)) <= 1e-13 * np.max(np.abs(V_ref))
+    W = W.reshape(cfg.n_mo, cfg.n_mo, cfg.n_pole)              # [m][p][s]
+    for s in (0, 1, 77, 199):
+        w_ref = oracle.residues(inp.B.numpy(), V_ref, s)       # [p][m]
+        assert np.max(np.abs(W[:, :, s].T - w_ref)) <= 1e-13 * np.max(np.abs(w_ref))
+    pkg.qsgw_sigma_destroy(plan)
+
+
+def test_general_occupations_and_unsorted_inputs():
+    cfg = qi.custom_config(40, 6, 20, n_pole=90, seed=9)
+    inp = qi.make_inputs(cfg)
+    g = torch.Generator().manual_seed(3)
+    inp.occ = torch.rand(cfg.n_mo, generator=g, dtype=torch.float64)          # fractional f_m: both terms of D
+    inp.occ[0], inp.occ[1] = 1.0, 0.0
+    inp.Omega = inp.Omega[torch.randperm(cfg.n_pole, generator=g)]            # sorting is not required
+    S, plan = _gpu_sigma(cfg, _to_dev(inp))
+    _assert_parity(S, _ref_sigma(cfg, inp))
+    _pkg().qsgw_sigma_destroy(plan)
+
+
+def test_exact_power_of_two_scaling_and_reproducibility():
+    pkg = _pkg()
+    cfg = qi.CONFIGS["tiny"]
+    inp = qi.make_inputs(cfg)
+    B, eps, occ, Om, Z = _to_dev(inp)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, 32)
+    S = pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta).clone()
+    S2 = pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta).clone()
+    assert torch.equal(S, S2), "same inputs, same plan: results must be bitwise reproducible"
+    assert torch.equal(pkg.qsgw_sigma_build(plan, B, eps, occ, Om, 2.0 * Z, cfg.eta), 4.0 * S)
+    assert torch.equal(pkg.qsgw_sigma_build(plan, 2.0 * B, eps, occ, Om, Z, cfg.eta), 16.0 * S)
+    pkg.qsgw_sigma_destroy(plan)
+
+
+def test_additive_over_pole_ranges_and_chunkings():
+    pkg = _pkg()
+    cfg = qi.custom_config(96, 12, 60, n_pole=700, seed=12)
+    inp = qi.make_inputs(cfg)
+    B, eps, occ, Om, Z = _to_dev(inp)
+    ref = _ref_sigma(cfg, inp)
+    scale = np.abs(ref).max()
+    results = []
+    for s_block in (0, 64, 250, 700):
+        S, plan = _gpu_sigma(cfg, (B, eps, occ, Om, Z), s_block=s_block)
+        _assert_parity(S, ref)
+        results.append(S.cpu().numpy())
+        pkg.qsgw_sigma_destroy(plan)
+    for r in results[1:]:
+        assert np.max(np.abs(r - results[0])) <= 1e-12 * scale
+    # streaming API over ragged ranges (pointer offsets into the full Z, ldz = full n_pole)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, 300, 128)
+    pkg.qsgw_sigma_begin(plan, B, eps, occ, cfg.eta)
+    for a, b in [(0, 1), (1, 300), (300, 555), (555, 700)]:
+        pkg.qsgw_sigma_add_poles(plan, Om[a:b], Z[:, a:b])
+    S = pkg.qsgw_sigma_finish(plan)
+    _assert_parity(S, ref)
+    # the one-shot call on a sub-range equals the oracle on that sub-range
+    S_r = pkg.qsgw_sigma_build(plan, B, eps, occ, Om[101:400], Z[:, 101:400], cfg.eta)
+    ref_r = oracle.sigma(inp.B.numpy(), inp.eps.numpy(), inp.occ.numpy(), inp.Omega.numpy()[101:400],
+                         inp.Z.numpy()[:, 101:400], cfg.eta, cfg.n_occ)
+    _assert_parity(S_r, ref_r)
+    pkg.qsgw_sigma_destroy(plan)
+
+
+def test_host_buffer_entry_point_matches_device_entry_point():
+    pkg = _pkg()
+    cfg = qi.custom_config(64, 10, 48, n_pole=540, s_block=128, seed=21)
+    inp = qi.make_inputs(cfg)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, cfg.s_block)
+    S_dev = pkg.qsgw_sigma_build(plan, *_to_dev(inp), cfg.eta)
+    torch.cuda.synchronize()
+    pinned = [t.pin_memory() for t in (inp.B, inp.eps, inp.occ, inp.Omega, inp.Z)]
+    S_host = pkg.qsgw_sigma_build_host(plan, *pinned, cfg.eta)
+    assert torch.equal(S_host, S_dev.cpu())
+    S_host2 = pkg.qsgw_sigma_build_host(plan, inp.B, inp.eps, inp.occ, inp.Omega, inp.Z, cfg.eta)   # pageable
+    assert torch.equal(S_host2, S_host)
+    _assert_parity(S_host, _ref_sigma(cfg, inp))
+    pkg.qsgw_sigma_destroy(plan)
+
+
+def test_null_case_and_error_codes():
+    pkg = _pkg()
+    cfg = qi.CONFIGS["tiny"]
+    inp = qi.make_inputs(cfg)
+    B, eps, occ, Om, Z = _to_dev(inp)
+    B0 = B.clone()
+    B0[:, :cfg.n_occ, cfg.n_occ:] = 0.0
+    B0[:, cfg.n_occ:, :cfg.n_occ] = 0.0
+    S, plan = _gpu_sigma(cfg, (B0, eps, occ, Om, Z))
+    assert torch.count_nonzero(S) == 0
+    with pytest.raises(pkg.QsgwSigmaError) as ei:
+        pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, 0.0)
+    assert ei.value.code == pkg.QSGW_SIGMA_ERR_INVALID_ARG
+    with pytest.raises(pkg.QsgwSigmaError):
+        pkg.qsgw_sigma_finish(plan)                           # finish without begin
+    with pytest.raises(pkg.QsgwSigmaError):
+        pkg.qsgw_sigma_add_poles(plan, Om, Z)                 # add_poles without begin
+    small_plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, 10)
+    with pytest.raises(pkg.QsgwSigmaError):
+        pkg.qsgw_sigma_build(small_plan, B, eps, occ, Om, Z, cfg.eta)   # n_pole > n_pole_max
+    # the plan is still usable after errors
+    S2 = pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta)
+    _assert_parity(S2, _ref_sigma(cfg, inp))
+    pkg.qsgw_sigma_destroy(plan)
+    pkg.qsgw_sigma_destroy(small_plan)
+
+
+def test_medium_config_full_parity():
+    cfg = qi.CONFIGS["medium"]
+    inp = qi.make_inputs(cfg)
+    S, plan = _gpu_sigma(cfg, _to_dev(inp))
+    _assert_parity(S, _ref_sigma(cfg, inp))
+    assert torch.equal(S, S.T)
+    _pkg().qsgw_sigma_destroy(plan)
