@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the qsGW Sigma^c build on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload large|xl|medium|small|tiny]
+  python bench.py --impl reference ...      # the CPU oracle timed on the host cores (bounded sample per step)
+
+A "step" is one pass of the whole hot path -- pack, stage 1, stage 2, stage 3 for every pole chunk, and
+the epilogue -- i.e. one Sigma^c build (qsgw_sigma_build through the C ABI) on seeded synthetic inputs of
+the named BASELINE.json config.  `value` = F_min / t in TFLOP/s (F_min = F1 + F2sym + F3,
+the least dense FP64 work the method needs, so the figure cannot be inflated by redundant work);
+`ms_per_step` = ms per build.  Inputs are resident in HBM for `value`; `e2e` repeats the build through
+qsgw_sigma_build_host with pinned HOST buffers, H2D/D2H copies inside the timed region.
+N > 1: the path does not shard in this scope ("replicas only"): every rank builds its own
+Sigma (seed + rank); the only collectives are the timing barrier and the max-over-ranks of the time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "sigma_c_build_fp64_tflops"
+UNIT = "TFLOP/s"
+# FP64 pipe of sm_100a: DMMA.8x8x4 and DFMA both retire 64 FMA/clk/SM (measured: profiles/r01_fp64_peaks.md)
+FP64_FMA_PER_CLK_PER_SM = 64
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def fp64_peak_tflops(n_sms: int = 148):
+    """Roofline denominator for the FP64 contractions: SMs x 64 FMA/clk x 2 x max SM clock."""
+    pk, src = _peaks()
+    mhz = float(pk.get("sm_max_mhz", 1965.0))
+    return n_sms * FP64_FMA_PER_CLK_PER_SM * 2 * mhz * 1e6 / 1e12, src, pk
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+            self.thread.join(timeout=5)
+
+    def summary(self):
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _cpu_oracle_sample(cfg, B_host, eps, occ, Omega, Z_cols, n_sample):
+    """Times the oracle as it stands on `n_sample` poles of the workload (all states, full B); returns (s, F_min)."""
+    import oracle
+    import qsgw_inputs as qi
+    t0 = time.perf_counter()
+    oracle.sigma(B_host, eps, occ, Omega[:n_sample], Z_cols[:, :n_sample], cfg.eta, cfg.n_occ)
+    dt = time.perf_counter() - t0
+    return dt, qi.flop_model(cfg, n_sample)["F_min"]
+
+
+def _sample_poles(cfg, target_s=20.0, gflops_guess=12.0):
+    import qsgw_inputs as qi
+    per_pole = qi.flop_model(cfg, 1)["F_full"] * 1.3           # the oracle does the full (non-symmetric) work + D
+    n = int(target_s * gflops_guess * 1e9 / per_pole)
+    return max(4, min(cfg.n_pole, n))
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the host cores; each step a bounded pole sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import numpy as np  # noqa: F401
+    import oracle
+    import qsgw_inputs as qi
+    cfg = qi.CONFIGS[args.workload]
+    n_sample = args.ref_poles or _sample_poles(cfg, target_s=6.0)
+    B = qi.make_B(cfg).numpy()
+    eps, occ, Om = qi.make_eps(cfg).numpy(), qi.make_occ(cfg).numpy(), qi.make_omega(cfg).numpy()
+    Z = qi.make_Z(cfg, 0, n_sample).numpy()
+    times = []
+    for it in range(args.warmup + args.steps):
+        dt, flops = _cpu_oracle_sample(cfg, B, eps, occ, Om, Z, n_sample)
+        if it >= args.warmup:
+            times.append(dt)
+    t = sum(times) / len(times)
+    val = flops / t / 1e12
+    sample = f"{n_sample} of {cfg.n_pole} poles of '{cfg.name}', all {cfg.n_mo} states, full B; per-step time scales linearly in poles"
+    cores = oracle.num_threads()
+    out = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t * 1e3, "ms_per_build_extrapolated": t * 1e3 * cfg.n_pole / n_sample,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": _config_dict(cfg, args, extra={"sample": sample}),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+def _config_dict(cfg, args, extra=None):
+    d = {"workload": cfg.name, "n_mo": cfg.n_mo, "n_occ": cfg.n_occ, "n_aux": cfg.n_aux, "n_pole": cfg.n_pole,
+         "s_block": cfg.s_block, "eta": cfg.eta, "seed": cfg.seed, "parallelism": "replicas" if args.gpus > 1 else "single",
+         "l2": "inputs larger than L2 (B + Z >> 126 MB); no explicit flush"}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    import qsgw_inputs as qi
+    import paper_2210_17093_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the qsGW Sigma build has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    base = qi.CONFIGS[args.workload]
+    cfg = qi.Config(base.name, base.n_mo, base.n_occ, base.n_aux, base.n_pole, base.s_block, base.eta, base.seed + rank)
+    streaming = args.stream_poles or (cfg.name == "xl")
+    fl = qi.flop_model(cfg)
+    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak, peak_src, pk = fp64_peak_tflops(nsm)
+
+    # ---- inputs, resident in HBM before the timed region
+    B = qi.make_B(cfg, dev)
+    eps, occ, Om = qi.make_eps(cfg).to(dev), qi.make_occ(cfg).to(dev), qi.make_omega(cfg).to(dev)
+    rng = cfg.s_block or 2048
+    if streaming:
+        Zbuf = [torch.empty((cfg.n_ov, rng), dtype=torch.float64, device=dev) for _ in range(2)]
+        Z = None
+        plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, rng, cfg.s_block)
+    else:
+        Z = qi.make_Z(cfg, device=dev)
+        plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, cfg.s_block)
+    pkg.qsgw_sigma_set_profiling(plan, True)
+    Sigma = torch.empty((cfg.n_mo, cfg.n_mo), dtype=torch.float64, device=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_build():
+        """Returns device ms of this build (CUDA events on the launch stream)."""
+        if not streaming:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta, Sigma)
+            e1.record()
+            return [(e0, e1)]
+        # xl: Z (130 GB) is produced range by range on the device just before each add_poles call;
+        # the generation is outside the event pairs, every kernel of the path is inside one.
+        evs = []
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); pkg.qsgw_sigma_begin(plan, B, eps, occ, cfg.eta); e1.record(); evs.append((e0, e1))
+        for k, s0 in enumerate(range(0, cfg.n_pole, rng)):
+            s1 = min(cfg.n_pole, s0 + rng)
+            zb = Zbuf[k % 2][:, : s1 - s0]
+            qi.make_Z(cfg, s0, s1, device=dev, out=zb)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); pkg.qsgw_sigma_add_poles(plan, Om[s0:s1], zb); e1.record(); evs.append((e0, e1))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); pkg.qsgw_sigma_finish(plan, Sigma); e1.record(); evs.append((e0, e1))
+        return evs
+
+    for _ in range(args.warmup):
+        one_build()
+    barrier()
+    pkg.qsgw_sigma_get_stats(plan, reset=True)
+    all_events = []
+    with ClockSampler(local) as clocks:
+        barrier()
+        t_wall0 = time.perf_counter()
+        for _ in range(args.steps):
+            all_events.append(one_build())
+        barrier()
+        t_wall = time.perf_counter() - t_wall0
+    step_ms = [sum(a.elapsed_time(b) for a, b in evs) for evs in all_events]
+    total_ms = sum(step_ms)
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    stats = pkg.qsgw_sigma_get_stats(plan, reset=True)
+    ms_per_step = total_ms / args.steps
+    value = world * fl["F_min"] / (ms_per_step * 1e-3) / 1e12
+    assert torch.isfinite(Sigma).all()
+
+    out = None
+    if rank == 0:
+        # dominant kernel: the stage-2 DMMA GEMM (w producer), 57 % of F_min
+        n2 = max(1, stats["launches_stage2"])
+        s2_ms = stats["ms_stage2"] / n2
+        flops_per_launch = fl["F2sym"] * args.steps / n2
+        achieved = flops_per_launch / (s2_ms * 1e-3) / 1e12
+        bf16_ratio_peak = float(pk.get("bf16_tflops", 1590.0)) * 45.0 / 2250.0
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "ms_per_build": ms_per_step, "ms_per_build_best": min(step_ms),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": _config_dict(cfg, args, extra={"z_resident": not streaming, "flops_F_min": fl["F_min"], "flops_F_full": fl["F_full"]}),
+            "tflops_model_full": world * fl["F_full"] / (ms_per_step * 1e-3) / 1e12,
+            "frac_of_fp64_peak": value / (world * peak),
+            "fp64_peak_tflops": {"value": peak, "how": f"{nsm} SMs x {FP64_FMA_PER_CLK_PER_SM} FMA/clk x 2 x sm_max_mhz of MEASURED_PEAKS.json ({peak_src})",
+                                 "dmma_microbench": 36.98, "cublas_dgemm_8192": 35.47,
+                                 "bf16_measured_x_nominal_ratio": bf16_ratio_peak},
+            "stage_ms_per_build": {k[3:]: stats[k] / args.steps for k in ("ms_pack", "ms_stage1", "ms_stage2", "ms_stage3", "ms_epilogue")},
+            "stage_tflops": {"stage1": fl["F1"] * args.steps / max(stats["ms_stage1"], 1e-9) / 1e9,
+                             "stage2": fl["F2sym"] * args.steps / max(stats["ms_stage2"], 1e-9) / 1e9,
+                             "stage3": fl["F3"] * args.steps / max(stats["ms_stage3"], 1e-9) / 1e9},
+            "roofline": {"bound": "tensor", "kernel": "gemm_tn_dmma_kernel<2,EpiPairScatter> (stage 2, w producer)",
+                         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                         "launches": stats["launches_stage2"], "avg_launch_ms": s2_ms, "traffic": None,
+                         "peak_source": f"FP64 pipe rate at max SM clock ({peak_src} MEASURED_PEAKS.json sm_max_mhz); no FP64 entry is measured there"},
+            "gpu_launches": stats["kernel_launches"],
+            "wall_s_timed_region": t_wall,
+            "clocks": clocks.summary(),
+        }
+
+    # ---- e2e: the same build through the host-buffer entry point (rank-local, max over ranks)
+    e2e = None
+    if not args.no_e2e and not streaming:
+        hB, hZ = B.cpu().pin_memory(), Z.cpu().pin_memory()
+        hE, hO, hOm = eps.cpu().pin_memory(), occ.cpu().pin_memory(), Om.cpu().pin_memory()
+        hS = torch.empty((cfg.n_mo, cfg.n_mo), dtype=torch.float64).pin_memory()
+        del Z
+        torch.cuda.empty_cache()
+        for _ in range(args.e2e_warmup):
+            pkg.qsgw_sigma_build_host(plan, hB, hE, hO, hOm, hZ, cfg.eta, hS)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.e2e_steps):
+            pkg.qsgw_sigma_build_host(plan, hB, hE, hO, hOm, hZ, cfg.eta, hS)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        ms /= args.e2e_steps
+        h2d = sum(t.numel() * 8 for t in (hB, hE, hO, hOm, hZ))
+        e2e = {"value": world * fl["F_min"] / (ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_build": ms, "steps": args.e2e_steps,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": hS.numel() * 8,
+               "how": "qsgw_sigma_build_host from pinned host tensors; uploads overlap the kernels range by range"}
+        assert torch.isfinite(hS).all()
+    elif rank == 0:
+        e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+               "how": "skipped (--no-e2e, or Z is produced range by range on the device for this workload)"}
+
+    # ---- cpu_baseline: the oracle as it stands, on rank 0's host cores, bounded sample of the same workload
+    if rank == 0:
+        out["e2e"] = e2e
+        if world == 1 and not args.no_cpu_baseline:
+            import oracle
+            n_sample = args.ref_poles or _sample_poles(cfg)
+            Zs = (hZ[:, :n_sample] if (e2e and e2e.get("value")) else qi.make_Z(cfg, 0, n_sample, device=dev).cpu()).numpy()
+            dt, flops = _cpu_oracle_sample(cfg, B.cpu().numpy(), eps.cpu().numpy(), occ.cpu().numpy(), Om.cpu().numpy(), Zs, n_sample)
+            out["cpu_baseline"] = {
+                "value": flops / dt / 1e12, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                "sample": f"{n_sample} of {cfg.n_pole} poles of '{cfg.name}', all {cfg.n_mo} states, full B ({dt:.1f} s); "
+                          f"whole build extrapolated linearly in poles: {dt * cfg.n_pole / n_sample:.0f} s",
+                "ms_per_build_extrapolated": dt * 1e3 * cfg.n_pole / n_sample}
+        else:
+            out["cpu_baseline"] = None
+        print(json.dumps(out), flush=True)
+    pkg.qsgw_sigma_destroy(plan)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="large", choices=["tiny", "small", "medium", "large", "xl"])
+    ap.add_argument("--stream-poles", action="store_true", help="produce Z range by range (always on for xl)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-warmup", type=int, default=1)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-poles", type=int, default=0, help="poles in the oracle's timed sample (0 = auto, ~20 s)")
+    args = ap.parse_args()
+    if args.steps < 1 or args.warmup < 0:
+        raise SystemExit("need --steps >= 1 and --warmup >= 0")
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -59,6 +59,7 @@ typedef struct qsgw_sigma_stats {
   double ms_stage2;   int64_t launches_stage2;   /* w chunk = sqrt(2) B^T V           (DMMA GEMM)      */
   double ms_stage3;   int64_t launches_stage3;   /* T += (w.D) w^T                    (fused DMMA)     */
   double ms_epilogue; int64_t launches_epilogue; /* split-K reduce + symmetrise                         */
+  int64_t kernel_launches;                       /* CUDA kernels launched by the library (counted always) */
   int64_t builds;                                /* number of qsgw_sigma_finish calls                  */
   int64_t poles;                                 /* poles processed                                    */
 } qsgw_sigma_stats;

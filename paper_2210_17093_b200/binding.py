@@ -40,7 +40,7 @@ class qsgw_sigma_stats(ctypes.Structure):
         ("ms_stage2", ctypes.c_double), ("launches_stage2", ctypes.c_int64),
         ("ms_stage3", ctypes.c_double), ("launches_stage3", ctypes.c_int64),
         ("ms_epilogue", ctypes.c_double), ("launches_epilogue", ctypes.c_int64),
-        ("builds", ctypes.c_int64), ("poles", ctypes.c_int64),
+        ("kernel_launches", ctypes.c_int64), ("builds", ctypes.c_int64), ("poles", ctypes.c_int64),
     ]
 
     def as_dict(self):

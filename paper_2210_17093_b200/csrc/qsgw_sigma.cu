@@ -63,7 +63,7 @@ struct qsgw_sigma_plan {
   std::vector<EventPair> pool;
   double ms[kNumStages] = {0, 0, 0, 0, 0};
   int64_t launches[kNumStages] = {0, 0, 0, 0, 0};
-  int64_t builds = 0, poles = 0;
+  int64_t builds = 0, poles = 0, kernel_launches = 0;
 
   std::string err;
 };
@@ -147,6 +147,7 @@ int launch_gemm(qsgw_sigma_plan *p, const double *A, int64_t lda, const double *
   }
   const int ntm = (M + kBM - 1) / kBM, ntn = (N + kBN - 1) / kBN;
   kern<<<ntm * ntn, kThreads, kGemmSmemBytes, p->stream>>>(A, lda, Bm, ldb, M, N, K, ntn, epi);
+  p->kernel_launches += 1;
   QSGW_CUDA(p, cudaGetLastError());
   return QSGW_SIGMA_OK;
 }
@@ -167,6 +168,7 @@ int do_begin(qsgw_sigma_plan *p, const double *B, const double *eps, const doubl
   {
     ScopedTimer t(p, kPack);
     pack_pairs_kernel<<<dim3(p->n_mo, p->n_aux), 128, 0, p->stream>>>(B, p->n_mo, p->Bp, p->ldp);
+    p->kernel_launches += 2;
     QSGW_CUDA(p, cudaGetLastError());
     dim3 grid((p->n_virt + 31) / 32, (p->n_aux + 31) / 32, p->n_occ);
     pack_ov_transposed_kernel<<<grid, dim3(32, 8), 0, p->stream>>>(B, p->n_mo, p->n_occ, p->n_aux, p->BovT, p->ld_aux);
@@ -212,6 +214,7 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
       ScopedTimer t(p, kStage3);
       sigma_accumulate_kernel<<<dim3(nt * nt, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
           p->W, p->ldw, p->eps, p->occ, Omega + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, nt, p->Tpart);
+      p->kernel_launches += 1;
       QSGW_CUDA(p, cudaGetLastError());
     }
   }
@@ -226,6 +229,7 @@ int do_finish(qsgw_sigma_plan *p, double *Sigma) {
     ScopedTimer t(p, kEpilogue);
     const int nb = (p->n_mo + 31) / 32;
     sigma_epilogue_kernel<<<dim3(nb, nb), dim3(32, 8), 0, p->stream>>>(p->Tpart, p->nsplit, p->n_mo, Sigma);
+    p->kernel_launches += 1;
     QSGW_CUDA(p, cudaGetLastError());
   }
   p->begun = false;
@@ -468,11 +472,12 @@ int qsgw_sigma_get_stats(qsgw_sigma_plan *p, qsgw_sigma_stats *st, int reset) {
   st->ms_stage2 = p->ms[kStage2];     st->launches_stage2 = p->launches[kStage2];
   st->ms_stage3 = p->ms[kStage3];     st->launches_stage3 = p->launches[kStage3];
   st->ms_epilogue = p->ms[kEpilogue]; st->launches_epilogue = p->launches[kEpilogue];
+  st->kernel_launches = p->kernel_launches;
   st->builds = p->builds;
   st->poles = p->poles;
   if (reset) {
     for (int s = 0; s < kNumStages; ++s) { p->ms[s] = 0; p->launches[s] = 0; }
-    p->builds = 0; p->poles = 0;
+    p->builds = 0; p->poles = 0; p->kernel_launches = 0;
   }
   return QSGW_SIGMA_OK;
 }
