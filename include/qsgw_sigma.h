@@ -146,6 +146,14 @@ int qsgw_sigma_get_stats(qsgw_sigma_plan *plan, qsgw_sigma_stats *stats, int res
  * INVALID_ARG if the block exceeds the array. */
 int qsgw_sigma_copy_workspace(qsgw_sigma_plan *plan, int which, double *dst, int64_t rows, int64_t cols);
 
+/* Measurement helper (no plan needed): times a register-resident FP64 loop on every SM of the current device and
+ * returns the achieved rate in *tflops (and the kernel time in *ms if non-NULL).  This is how the FP64 roofline
+ * denominator (SMs x 64 FMA/clk x 2 x SM clock) is checked on the box, MEASURED_PEAKS.json having no FP64 entry.
+ *   mode 0: DMMA.8x8x4 only   1: DFMA only   2: 32 DMMA + `mix` DFMA per iteration (mix a multiple of 8)
+ *   mode 3: DMMA fed by LDS.64 fragment loads (the GEMM inner loop without global traffic)
+ * iters >= 1 loop iterations per warp; ctas_per_sm >= 1 CTAs of 256 threads per SM.  Synchronises the stream. */
+int qsgw_sigma_fp64_probe(int mode, int iters, int mix, int ctas_per_sm, void *cuda_stream, double *tflops, double *ms);
+
 /* Library version (major*10000 + minor*100 + patch). */
 int qsgw_sigma_version(void);
 

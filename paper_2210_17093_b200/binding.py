@@ -23,7 +23,7 @@ QSGW_SIGMA_ERR_CUDA = -3
 EXPORTS = (
     "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
     "qsgw_sigma_build_host", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
-    "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_copy_workspace", "qsgw_sigma_version",
+    "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_copy_workspace", "qsgw_sigma_version", "qsgw_sigma_fp64_probe",
 )
 
 
@@ -84,6 +84,8 @@ def load_library() -> ctypes.CDLL:
         lib.qsgw_sigma_get_stats.argtypes = [vp, ctypes.POINTER(qsgw_sigma_stats), ci]
         lib.qsgw_sigma_copy_workspace.restype = ci
         lib.qsgw_sigma_copy_workspace.argtypes = [vp, ci, dp, i64, i64]
+        lib.qsgw_sigma_fp64_probe.restype = ci
+        lib.qsgw_sigma_fp64_probe.argtypes = [ci, ci, ci, ci, vp, ctypes.POINTER(cd), ctypes.POINTER(cd)]
         lib.qsgw_sigma_version.restype = ci
         lib.qsgw_sigma_version.argtypes = []
         _lib = lib
@@ -238,6 +240,17 @@ def qsgw_sigma_copy_workspace(plan: Plan, which: int, rows: int, cols: int) -> t
     _check(load_library().qsgw_sigma_copy_workspace(plan.handle, int(which), out.data_ptr(), int(rows), int(cols)),
            plan.handle)
     return out
+
+
+def qsgw_sigma_fp64_probe(mode: int, iters: int = 20000, mix: int = 0, ctas_per_sm: int = 1) -> dict:
+    """Measured FP64 issue rate of the current device (mode 0 DMMA, 1 DFMA, 2 DMMA+DFMA mix, 3 LDS-fed DMMA)."""
+    tf, ms = ctypes.c_double(), ctypes.c_double()
+    sptr = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    rc = load_library().qsgw_sigma_fp64_probe(int(mode), int(iters), int(mix), int(ctas_per_sm), sptr,
+                                              ctypes.byref(tf), ctypes.byref(ms))
+    if rc != QSGW_SIGMA_OK:
+        raise QsgwSigmaError(rc, "fp64 probe failed")
+    return {"tflops": tf.value, "ms": ms.value}
 
 
 def qsgw_sigma_version() -> int:

@@ -7,7 +7,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libqsgw_sigma.so")
-SOURCES = ["qsgw_sigma.cu"]
+SOURCES = ["qsgw_sigma.cu", "fp64_probe.cu"]
 HEADERS = ["dmma_gemm.cuh", "sigma_kernels.cuh", os.path.join("..", "..", "include", "qsgw_sigma.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

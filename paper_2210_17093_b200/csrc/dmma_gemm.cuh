@@ -1,23 +1,31 @@
-// dmma_gemm.cuh -- FP64 tensor-core (DMMA) building blocks and the "TN" GEMM used by stages 1 and 2.
+// dmma_gemm.cuh -- FP64 tensor-core (DMMA) building blocks and the warp-specialised "TN" GEMM of stages 1 and 2.
 //
-// sm_100a has no tcgen05 kind for f64 (CUDA 12.9 lists f16/tf32/i8/f8f6f4/mx* only), so FP64
-// contractions go through mma.sync.m8n8k4.f64, which assembles to DMMA.8x8x4.  Accumulators live in
-// registers; operand tiles are staged global -> shared with a 4-deep cp.async (LDGSTS) ring and read
-// as LDS.64 fragments from padded, bank-conflict-free layouts.  Measured on B200: an LDS-fed 64x32
-// warp tile sustains 36.98 TFLOP/s = 99 % of 148 SM x 64 FMA/clk x 1.965 GHz (profiles/r01_fp64_peaks.md).
+// sm_100a has no tcgen05 kind for f64 (CUDA 12.9 lists f16/tf32/i8/f8f6f4/mx* only), so FP64 contractions go
+// through mma.sync.m8n8k4.f64, which assembles to DMMA.8x8x4 (256 FMA; 64 FMA/clk/SM).  Accumulators live in
+// registers.  A CTA is 12 warps: 8 consumer warps (2 x 4, each a 64 x 32 warp tile of 8 x 4 DMMA fragments,
+// fragments interleaved across warps so that ragged edge tiles shed work evenly) that do nothing but
+// LDS.64 fragment loads + DMMA, and 4 producer warps (one per SM sub-partition) that stage the operand tiles
+// global -> shared with cp.async (LDGSTS).  The two roles meet only through mbarriers (full[stage] /
+// empty[stage]); there is no CTA-wide barrier in the main loop, so the DMMA pipe never drains at a k-tile edge.
+// Registers are re-split with setmaxnreg (consumers up, producers down).  Shared tiles are padded so that every
+// fragment load is bank-conflict free.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace qsgw {
 
-constexpr int kThreads = 256;   // 8 warps: 2 (M) x 4 (N), warp tile 64 x 32
+constexpr int kConsumerWarps = 8;                    // 2 (M) x 4 (N)
+constexpr int kProducerWarps = 4;
+constexpr int kConsumerThreads = kConsumerWarps * 32;
+constexpr int kProducerThreads = kProducerWarps * 32;
+constexpr int kThreads = kConsumerThreads + kProducerThreads;   // 384
 constexpr int kBM = 128;
 constexpr int kBN = 128;
 constexpr int kBK = 16;
-constexpr int kStages = 4;
 constexpr int kLdT = kBM + 4;   // k-major tile rows [k][128 + 4]: ld = 4 (mod 16) doubles -> LDS.64 fragments conflict-free
 constexpr int kLdK = kBK + 4;   // row-major tile rows [row][16 + 4]: same property for the [row][k] layout of stage 3
+constexpr int kGemmStages = 6;
 
 // D(2 regs) += A(8x4, row) * B(4x8, col); lane holds A[lane/4][lane%4], B[lane%4][lane/4],
 // D[lane/4][2*(lane%4) + {0,1}].
@@ -27,43 +35,139 @@ __device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) 
       : "d"(a), "d"(b));
 }
 
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
 __device__ __forceinline__ void cp_async_16(void *smem_dst, const void *gmem_src, int src_bytes) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem_src), "r"(src_bytes) : "memory");
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(src_bytes)
+               : "memory");
 }
 __device__ __forceinline__ void cp_async_8(void *smem_dst, const void *gmem_src, int src_bytes) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(s), "l"(gmem_src), "r"(src_bytes) : "memory");
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(src_bytes)
+               : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// ---- mbarrier pipeline primitives (shared::cta)
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// one arrival on `bar` once all cp.async issued so far by this thread have landed (not counted as pending: the
+// barrier's init count includes it)
+__device__ __forceinline__ void cp_async_mbar_arrive_noinc(uint64_t *bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+template <int R>
+__device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R)); }
+template <int R>
+__device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(R)); }
+
+// Fragment geometry of consumer warp `warp` (0..7) and lane: warp (wmi, wni) = (warp & 1, warp >> 1) owns the
+// 8-row blocks 2i + wmi (i < 8) and the 8-column blocks 4j + wni (j < 4) of the 128 x 128 CTA tile.
+struct FragMap {
+  int wmi, wni, g, t;      // g = lane / 4 (fragment row / column), t = lane % 4 (k within a k4 step)
+  int mi_cnt, nj_cnt;      // fragments of this warp that hold at least one valid row / column (warp-uniform)
+  __device__ __forceinline__ FragMap(int warp, int lane, int rows_valid, int cols_valid) {
+    wmi = warp & 1; wni = warp >> 1; g = lane >> 2; t = lane & 3;
+    const int rb = min(16, (max(rows_valid, 0) + 7) >> 3), cb = min(16, (max(cols_valid, 0) + 7) >> 3);
+    mi_cnt = max(0, (rb - wmi + 1) >> 1);
+    nj_cnt = max(0, (cb - wni + 3) >> 2);
+  }
+  __device__ __forceinline__ int row(int i) const { return 16 * i + 8 * wmi + g; }          // of fragment i, this lane's A row
+  __device__ __forceinline__ int col(int j) const { return 32 * j + 8 * wni + g; }          // of fragment j, this lane's B column
+  __device__ __forceinline__ int out_col(int j) const { return 32 * j + 8 * wni + 2 * t; }  // first of this lane's 2 accumulator columns
+};
+
+// One k-tile (16 deep) of DMMA work on k-major tiles As[k][kLdT], Bs[k][kLdT].
+template <bool FULL>
+__device__ __forceinline__ void mma_ktile_kmajor(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
+  const double *ap = as + 8 * fm.wmi + fm.g + fm.t * kLdT;
+  const double *bp = bs + 8 * fm.wni + fm.g + fm.t * kLdT;
+#pragma unroll
+  for (int kk = 0; kk < kBK / 4; ++kk) {
+    double a[8], b[4];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      if (FULL || i < fm.mi_cnt) a[i] = ap[kk * 4 * kLdT + 16 * i];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if (FULL || j < fm.nj_cnt) b[j] = bp[kk * 4 * kLdT + 32 * j];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      if (FULL || i < fm.mi_cnt) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          if (FULL || j < fm.nj_cnt) dmma_m8n8k4(acc[i][j], a[i], b[j]);
+      }
+  }
 }
 
-// Stage one k-major operand tile: dst[k][c] = src[k*ld + c], k < kBK, c < 128; rows >= kvalid and
-// columns >= cvalid are zero-filled.  VEC = doubles per cp.async (2 needs 16-byte aligned src rows).
+// Same on row-major tiles As[row][kLdK], Bs[row][kLdK] (stage 3).
+template <bool FULL>
+__device__ __forceinline__ void mma_ktile_rowmajor(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
+  const double *ap = as + (8 * fm.wmi + fm.g) * kLdK + fm.t;
+  const double *bp = bs + (8 * fm.wni + fm.g) * kLdK + fm.t;
+#pragma unroll
+  for (int kk = 0; kk < kBK / 4; ++kk) {
+    double a[8], b[4];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      if (FULL || i < fm.mi_cnt) a[i] = ap[16 * i * kLdK + 4 * kk];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if (FULL || j < fm.nj_cnt) b[j] = bp[32 * j * kLdK + 4 * kk];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      if (FULL || i < fm.mi_cnt) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          if (FULL || j < fm.nj_cnt) dmma_m8n8k4(acc[i][j], a[i], b[j]);
+      }
+  }
+}
+
+// Producer side: stage one k-major operand tile dst[k][c] = src[k*ld + c], k < kBK, c < 128, with the 128 producer
+// threads (pt = 0..127); rows >= kvalid and columns >= cvalid are zero-filled.  VEC = doubles per cp.async
+// (2 needs 16-byte aligned src rows).
 template <int VEC>
 __device__ __forceinline__ void load_tile_kmajor(double *dst, const double *src, int64_t ld, int kvalid, int cvalid,
-                                                 const double *safe) {
-  const int tid = threadIdx.x;
+                                                 const double *safe, int pt) {
   if (VEC == 2) {
+    const int c = (pt & 63) * 2, r0 = pt >> 6;
+    int n = cvalid - c;
+    n = n < 0 ? 0 : (n > 2 ? 2 : n);
+    const double *s = src + (int64_t)r0 * ld + c;
+    double *d = dst + r0 * kLdT + c;
 #pragma unroll
-    for (int j = 0; j < (kBK * kBM / 2) / kThreads; ++j) {
-      const int id = tid + j * kThreads;
-      const int r = id >> 6, c = (id & 63) * 2;
-      int n = cvalid - c;
-      n = n < 0 ? 0 : (n > 2 ? 2 : n);
-      const int nb = (r < kvalid) ? n * 8 : 0;
-      cp_async_16(dst + r * kLdT + c, nb ? src + (int64_t)r * ld + c : safe, nb);
+    for (int j = 0; j < kBK / 2; ++j) {
+      const int nb = (r0 + 2 * j < kvalid) ? n * 8 : 0;
+      cp_async_16(d + 2 * j * kLdT, nb ? s + (int64_t)(2 * j) * ld : safe, nb);
     }
   } else {
+    const int c = pt;
+    const int nbc = (c < cvalid) ? 8 : 0;
+    const double *s = src + c;
+    double *d = dst + c;
 #pragma unroll
-    for (int j = 0; j < (kBK * kBM) / kThreads; ++j) {
-      const int id = tid + j * kThreads;
-      const int r = id >> 7, c = id & 127;
-      const int nb = (r < kvalid && c < cvalid) ? 8 : 0;
-      cp_async_8(dst + r * kLdT + c, nb ? src + (int64_t)r * ld + c : safe, nb);
+    for (int r = 0; r < kBK; ++r) {
+      const int nb = (r < kvalid) ? nbc : 0;
+      cp_async_8(d + r * kLdT, nb ? s + (int64_t)r * ld : safe, nb);
     }
   }
 }
@@ -109,72 +213,82 @@ struct EpiPairScatter {
   }
 };
 
-constexpr size_t kGemmSmemBytes = (size_t)kStages * 2 * kBK * kLdT * sizeof(double);
+constexpr size_t kGemmSmemBytes = (size_t)kGemmStages * 2 * kBK * kLdT * sizeof(double) + 2 * kGemmStages * sizeof(uint64_t);
 
 // C(M x N) = epilogue( sum_k A[k][m] * B[k][n] ),  A stored [K][lda] (m contiguous), B stored [K][ldb] (n contiguous).
 // A must be 16-byte aligned with even lda (library workspace); B may be arbitrary when VECB == 1.
-// grid.x = ceil(M/128) * ceil(N/128), n-tile fastest so CTAs that share an A tile run together.
+// grid.x = ntm * ntn tiles of 128 x 128; m_fastest picks which tile index varies fastest (the dimension with fewer
+// tiles, so that concurrently running CTAs share operand panels in L2).
 template <int VECB, class Epi>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_tn_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__restrict__ Bm, int64_t ldb, int M, int N,
-                    int K, int ntn, Epi epi) {
+                    int K, int ntm, int ntn, int m_fastest, Epi epi) {
   extern __shared__ __align__(16) double smem[];
   double *As = smem;
-  double *Bs = smem + kStages * kBK * kLdT;
+  double *Bs = smem + kGemmStages * kBK * kLdT;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + 2 * kGemmStages * kBK * kLdT);
+  uint64_t *empty = full + kGemmStages;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tm = blockIdx.x / ntn, tn = blockIdx.x - tm * ntn;
+  int tm, tn;
+  if (m_fastest) { tn = blockIdx.x / ntm; tm = blockIdx.x - tn * ntm; }
+  else { tm = blockIdx.x / ntn; tn = blockIdx.x - tm * ntn; }
   const int m0 = tm * kBM, n0 = tn * kBN;
-  const int wm = (warp & 1) * 64, wn = (warp >> 1) * 32;
   const int KT = (K + kBK - 1) / kBK;
 
-  auto issue = [&](int kt) {
-    if (kt < KT) {
-      const int st = kt % kStages, k0 = kt * kBK;
-      load_tile_kmajor<2>(As + st * kBK * kLdT, A + (int64_t)k0 * lda + m0, lda, K - k0, M - m0, A);
-      load_tile_kmajor<VECB>(Bs + st * kBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, K - k0, N - n0, Bm);
+  if (tid == 0) {
+    for (int s = 0; s < kGemmStages; ++s) {
+      mbar_init(full + s, kProducerThreads);
+      mbar_init(empty + s, kConsumerWarps);
     }
-    cp_async_commit();
-  };
-
-  double acc[8][4][2];
-#pragma unroll
-  for (int i = 0; i < 8; ++i)
-#pragma unroll
-    for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-#pragma unroll
-  for (int s = 0; s < kStages - 1; ++s) issue(s);
-
-  for (int kt = 0; kt < KT; ++kt) {
-    cp_async_wait<kStages - 2>();
-    __syncthreads();
-    issue(kt + kStages - 1);
-    const double *as = As + (kt % kStages) * kBK * kLdT + wm + (lane >> 2);
-    const double *bs = Bs + (kt % kStages) * kBK * kLdT + wn + (lane >> 2);
-#pragma unroll
-    for (int kk = 0; kk < kBK / 4; ++kk) {
-      const int k = kk * 4 + (lane & 3);
-      double a[8], b[4];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) a[i] = as[k * kLdT + 8 * i];
-#pragma unroll
-      for (int j = 0; j < 4; ++j) b[j] = bs[k * kLdT + 8 * j];
-#pragma unroll
-      for (int i = 0; i < 8; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) dmma_m8n8k4(acc[i][j], a[i], b[j]);
-    }
+    mbar_fence_init();
   }
-  cp_async_wait<0>();
+  __syncthreads();
 
+  if (warp >= kConsumerWarps) {
+    // ------------------------------------------------ producers: cp.async the k-tiles into the ring
+    reg_dec<40>();
+    const int pt = tid - kConsumerThreads;
+    int st = 0;
+    uint32_t ph = 1;   // a fresh barrier passes a wait on parity 1: the first pass over the ring does not block
+    for (int kt = 0; kt < KT; ++kt) {
+      mbar_wait(empty + st, ph);
+      const int k0 = kt * kBK;
+      load_tile_kmajor<2>(As + st * kBK * kLdT, A + (int64_t)k0 * lda + m0, lda, K - k0, M - m0, A, pt);
+      load_tile_kmajor<VECB>(Bs + st * kBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, K - k0, N - n0, Bm, pt);
+      cp_async_mbar_arrive_noinc(full + st);
+      if (++st == kGemmStages) { st = 0; ph ^= 1; }
+    }
+    cp_async_wait_all();
+  } else {
+    // ------------------------------------------------ consumers: LDS.64 fragments + DMMA
+    reg_inc<232>();
+    const FragMap fm(warp, lane, M - m0, N - n0);
+    const bool full_tile = fm.mi_cnt == 8 && fm.nj_cnt == 4;
+    double acc[8][4][2];
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const int row = m0 + wm + 8 * i + (lane >> 2);
-    if (row < M) {
+    for (int i = 0; i < 8; ++i)
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const int col = n0 + wn + 8 * j + 2 * (lane & 3);
-        if (col < N) epi(row, col, acc[i][j][0], acc[i][j][1], N);
+      for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    int st = 0;
+    uint32_t ph = 0;
+#pragma unroll 1
+    for (int kt = 0; kt < KT; ++kt) {
+      mbar_wait(full + st, ph);
+      if (full_tile) mma_ktile_kmajor<true>(acc, As + st * kBK * kLdT, Bs + st * kBK * kLdT, fm);
+      else mma_ktile_kmajor<false>(acc, As + st * kBK * kLdT, Bs + st * kBK * kLdT, fm);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty + st);
+      if (++st == kGemmStages) { st = 0; ph ^= 1; }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int row = m0 + fm.row(i);
+      if (row < M) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int col = n0 + fm.out_col(j);
+          if (col < N) epi(row, col, acc[i][j][0], acc[i][j][1], N);
+        }
       }
     }
   }

@@ -35,6 +35,7 @@ struct qsgw_sigma_plan {
   int n_mo = 0, n_occ = 0, n_virt = 0, n_aux = 0;
   int64_t n_ov = 0, n_pole_max = 0;
   int s_chunk = 0;
+  int64_t v_cols = 0;   // poles per stage-1 launch (V holds this many columns)
   cudaStream_t stream = nullptr;
   int device = 0;
 
@@ -146,7 +147,9 @@ int launch_gemm(qsgw_sigma_plan *p, const double *A, int64_t lda, const double *
     configured = true;
   }
   const int ntm = (M + kBM - 1) / kBM, ntn = (N + kBN - 1) / kBN;
-  kern<<<ntm * ntn, kThreads, kGemmSmemBytes, p->stream>>>(A, lda, Bm, ldb, M, N, K, ntn, epi);
+  if ((int64_t)ntm * ntn > INT32_MAX) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "GEMM grid too large");
+  // the dimension with fewer tiles varies fastest: the CTAs of one wave then share its few operand panels in L2
+  kern<<<ntm * ntn, kThreads, kGemmSmemBytes, p->stream>>>(A, lda, Bm, ldb, M, N, K, ntm, ntn, ntm <= ntn ? 1 : 0, epi);
   p->kernel_launches += 1;
   QSGW_CUDA(p, cudaGetLastError());
   return QSGW_SIGMA_OK;
@@ -193,29 +196,33 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
     sigma_configured = true;
   }
   const int nt = (p->n_mo + kBM - 1) / kBM;
-  for (int64_t c0 = 0; c0 < n_pole; c0 += p->s_chunk) {
-    const int sc = (int)std::min<int64_t>(p->s_chunk, n_pole - c0);
-    const double *Zc = Z + c0;
-    {  // stage 1: V[P][s] = sum_ia BovT[ia][P] * Z[ia][c0+s]
+  for (int64_t v0 = 0; v0 < n_pole; v0 += p->v_cols) {
+    const int64_t nv = std::min<int64_t>(p->v_cols, n_pole - v0);
+    {  // stage 1 for all poles of this range at once (enough tiles to fill the SMs evenly):
+       // V[P][s] = sum_ia BovT[ia][P] * Z[ia][v0+s]
       ScopedTimer t(p, kStage1);
       EpiStore epi{p->V, p->ldv, 1.0};
+      const double *Zc = Z + v0;
       int rc = aligned16(Zc, ldz)
-                   ? launch_gemm<2>(p, p->BovT, p->ld_aux, Zc, ldz, p->n_aux, sc, (int)p->n_ov, epi)
-                   : launch_gemm<1>(p, p->BovT, p->ld_aux, Zc, ldz, p->n_aux, sc, (int)p->n_ov, epi);
+                   ? launch_gemm<2>(p, p->BovT, p->ld_aux, Zc, ldz, p->n_aux, (int)nv, (int)p->n_ov, epi)
+                   : launch_gemm<1>(p, p->BovT, p->ld_aux, Zc, ldz, p->n_aux, (int)nv, (int)p->n_ov, epi);
       if (rc) return rc;
     }
-    {  // stage 2: w[(p<=m)][s] = sqrt(2) sum_P Bp[P][(p,m)] * V[P][s], scattered to W[(m,p)] and W[(p,m)]
-      ScopedTimer t(p, kStage2);
-      EpiPairScatter epi{p->W, p->ldw, p->pairs, p->n_mo, std::sqrt(2.0)};
-      int rc = launch_gemm<2>(p, p->Bp, p->ldp, p->V, p->ldv, (int)p->n_pair, sc, p->n_aux, epi);
-      if (rc) return rc;
-    }
-    {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
-      ScopedTimer t(p, kStage3);
-      sigma_accumulate_kernel<<<dim3(nt * nt, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
-          p->W, p->ldw, p->eps, p->occ, Omega + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, nt, p->Tpart);
-      p->kernel_launches += 1;
-      QSGW_CUDA(p, cudaGetLastError());
+    for (int64_t c0 = 0; c0 < nv; c0 += p->s_chunk) {
+      const int sc = (int)std::min<int64_t>(p->s_chunk, nv - c0);
+      {  // stage 2: w[(p<=m)][s] = sqrt(2) sum_P Bp[P][(p,m)] * V[P][c0+s], scattered to W[(m,p)] and W[(p,m)]
+        ScopedTimer t(p, kStage2);
+        EpiPairScatter epi{p->W, p->ldw, p->pairs, p->n_mo, std::sqrt(2.0)};
+        int rc = launch_gemm<2>(p, p->Bp, p->ldp, p->V + c0, p->ldv, (int)p->n_pair, sc, p->n_aux, epi);
+        if (rc) return rc;
+      }
+      {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
+        ScopedTimer t(p, kStage3);
+        sigma_accumulate_kernel<<<dim3(nt * nt, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
+            p->W, p->ldw, p->eps, p->occ, Omega + v0 + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, nt, p->Tpart);
+        p->kernel_launches += 1;
+        QSGW_CUDA(p, cudaGetLastError());
+      }
     }
   }
   p->poles += n_pole;
@@ -302,7 +309,11 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
   p->n_pair = (int64_t)n_mo * (n_mo + 1) / 2;
   p->ldp = round_up(p->n_pair, 2);
   p->ld_aux = round_up(n_aux, 2);
-  p->ldv = round_up(p->s_chunk, 2);
+  {  // V holds as many poles as fit in 4 GiB (whole chunks), at most n_pole_max
+    const int64_t cap = std::max<int64_t>(1, ((int64_t)4 << 30) / (8 * (int64_t)n_aux) / p->s_chunk) * p->s_chunk;
+    p->v_cols = std::min<int64_t>(round_up(n_pole_max, 2), cap);
+  }
+  p->ldv = round_up(p->v_cols, 2);
   p->ldw = round_up(p->s_chunk, 2);
   // split-K of stage 3 over the internal state m: enough CTAs for >= ~16 waves of the SMs, at most N splits
   const int nt = (n_mo + kBM - 1) / kBM;

@@ -53,15 +53,29 @@ __global__ void pack_ov_transposed_kernel(const double *__restrict__ B, int n_mo
 // ---------------------------------------------------------------- stage 3
 // D(m,s,omega) = occ_m * x1/(x1^2+eta^2) + (1-occ_m) * x2/(x2^2+eta^2),  x1 = (omega-eps_m)+Omega_s,
 // x2 = (omega-eps_m)-Omega_s: real part of the two terms of Eq. (17).  d = omega - eps_m.
-__device__ __forceinline__ double lehmann_term(double x, double eta2) { return x / fma(x, x, eta2); }
+// x/(x^2+eta^2) without the IEEE division's slow path: MUFU.RCP64H seed + two Newton steps folded into the
+// quotient (relative error ~2 ulp; x^2+eta^2 >= eta^2 > 0 is never subnormal for physical energies).
+__device__ __forceinline__ double lehmann_term(double x, double eta2) {
+  const double y = fma(x, x, eta2);
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
+  double e = fma(-y, r, 1.0);
+  r = fma(r, e, r);
+  const double q = x * r;
+  e = fma(-y, r, 1.0);
+  return fma(q, e, q);
+}
 
+// OCC: 1 = f_m == 1 (occupied), 0 = f_m == 0 (virtual), 2 = fractional (both terms)
+template <int OCC>
 __device__ __forceinline__ double denominator_D(double d, double Omega_s, double occ_m, double eta2) {
-  if (occ_m == 1.0) return lehmann_term(d + Omega_s, eta2);
-  if (occ_m == 0.0) return lehmann_term(d - Omega_s, eta2);
+  if (OCC == 1) return lehmann_term(d + Omega_s, eta2);
+  if (OCC == 0) return lehmann_term(d - Omega_s, eta2);
   return occ_m * lehmann_term(d + Omega_s, eta2) + (1.0 - occ_m) * lehmann_term(d - Omega_s, eta2);
 }
 
-constexpr size_t kSigmaSmemBytes = (size_t)kStages * 2 * kBM * kLdK * sizeof(double);
+constexpr int kSigmaStages = 5;
+constexpr size_t kSigmaSmemBytes = (size_t)kSigmaStages * 2 * kBM * kLdK * sizeof(double) + 2 * kSigmaStages * sizeof(uint64_t);
 
 // One CTA: output tile (tp, tq) of T, 128 x 128, for the internal states m in [z*m_per_split, ...) and all
 // s_c poles of the chunk.  k-tiles of 16 poles at fixed m, so eps_m / occ_m are CTA-uniform per k-tile.
@@ -69,123 +83,172 @@ constexpr size_t kSigmaSmemBytes = (size_t)kStages * 2 * kBM * kLdK * sizeof(dou
 //   Omega [s_c]       excitation energies of the chunk
 //   Tpart [nsplit][N][N]  split-K partial tiles; slot z is owned by the CTAs with blockIdx.y == z and is
 //                     read-modify-written once per launch -> accumulation order is fixed, results reproducible.
+// Roles: the 4 producer warps form the operands -- the q rows of w go global -> shared by cp.async untouched, the
+// p rows go global -> registers (prefetched one k-tile ahead), are multiplied by D(m, s, eps_p) and stored to
+// shared: the scaled operand A = w.D exists only in shared memory.  The 8 consumer warps run LDS + DMMA only.
 __global__ void __launch_bounds__(kThreads, 1)
 sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double *__restrict__ eps,
                         const double *__restrict__ occ, const double *__restrict__ Omega, int n_mo, int s_c,
                         double eta2, int m_per_split, int ntq, double *__restrict__ Tpart) {
   extern __shared__ __align__(16) double smem[];
-  double *As = smem;                             // [stage][128][kLdK]  p rows, scaled in place by D
-  double *Bs = smem + kStages * kBM * kLdK;      // [stage][128][kLdK]  q rows, raw
+  double *As = smem;                                  // [stage][128][kLdK]  p rows, already scaled by D
+  double *Bs = smem + kSigmaStages * kBM * kLdK;      // [stage][128][kLdK]  q rows, raw
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + 2 * kSigmaStages * kBM * kLdK);
+  uint64_t *empty = full + kSigmaStages;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int tp = blockIdx.x / ntq, tq = blockIdx.x - tp * ntq;
   const int p0 = tp * kBM, q0 = tq * kBN;
-  const int wm = (warp & 1) * 64, wn = (warp >> 1) * 32;
   const int m_begin = blockIdx.y * m_per_split;
   const int m_end = min(n_mo, m_begin + m_per_split);
   const int KTS = (s_c + kBK - 1) / kBK;         // k-tiles per m
   const int KT = (m_end - m_begin) * KTS;
 
-  // ---- loader: thread owns 4 (row, 16-byte chunk) slots of each operand tile; counters (m, ks) advance per k-tile
-  int ld_m = m_begin, ld_ks = 0;
-  auto issue = [&](int kt) {
-    if (kt < KT) {
-      const int st = kt % kStages;
-      const int s0 = ld_ks * kBK;
-      const double *wm_base = W + (int64_t)ld_m * n_mo * ldw + s0;
-#pragma unroll
-      for (int j = 0; j < (kBM * kBK / 2) / kThreads; ++j) {
-        const int id = tid + j * kThreads;
-        const int r = id >> 3, c = (id & 7) * 2;
-        int n = s_c - s0 - c;
-        n = n < 0 ? 0 : (n > 2 ? 2 : n);
-        const int nbA = (p0 + r < n_mo) ? n * 8 : 0;
-        const int nbB = (q0 + r < n_mo) ? n * 8 : 0;
-        cp_async_16(As + (st * kBM + r) * kLdK + c, nbA ? wm_base + (int64_t)(p0 + r) * ldw + c : W, nbA);
-        cp_async_16(Bs + (st * kBM + r) * kLdK + c, nbB ? wm_base + (int64_t)(q0 + r) * ldw + c : W, nbB);
-      }
-      if (++ld_ks == KTS) { ld_ks = 0; ++ld_m; }
+  if (tid == 0) {
+    for (int s = 0; s < kSigmaStages; ++s) {
+      mbar_init(full + s, 2 * kProducerThreads);   // per producer thread: one cp.async arrival (B tile) + one plain arrival (A tile)
+      mbar_init(empty + s, kConsumerWarps);
     }
-    cp_async_commit();
-  };
-
-  // ---- operand producer: thread scales 8 consecutive k of one p row, A[p][k] *= D(m, s0+k, eps_p)
-  const int sc_row = tid >> 1, sc_k = (tid & 1) * 8;
-  const double eps_p = (p0 + sc_row < n_mo) ? __ldg(eps + p0 + sc_row) : 0.0;
-  int sc_m = m_begin, sc_ks = 0;
-  auto scale = [&](int kt) {
-    if (kt < KT) {
-      const int st = kt % kStages;
-      const int s0 = sc_ks * kBK + sc_k;
-      const double d = eps_p - __ldg(eps + sc_m);
-      const double f = __ldg(occ + sc_m);
-      double2 *row = reinterpret_cast<double2 *>(As + (st * kBM + sc_row) * kLdK + sc_k);
-#pragma unroll
-      for (int h = 0; h < 4; ++h) {
-        const int s = s0 + 2 * h;
-        const double om0 = (s < s_c) ? __ldg(Omega + s) : 1.0;
-        const double om1 = (s + 1 < s_c) ? __ldg(Omega + s + 1) : 1.0;
-        double2 wv = row[h];
-        wv.x *= denominator_D(d, om0, f, eta2);
-        wv.y *= denominator_D(d, om1, f, eta2);
-        row[h] = wv;
-      }
-      if (++sc_ks == KTS) { sc_ks = 0; ++sc_m; }
-    }
-  };
-
-  double acc[8][4][2];
-#pragma unroll
-  for (int i = 0; i < 8; ++i)
-#pragma unroll
-    for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-#pragma unroll
-  for (int s = 0; s < kStages - 1; ++s) issue(s);
-  cp_async_wait<kStages - 2>();   // k-tile 0 landed (this thread's copies)
-  __syncthreads();
-  scale(0);
-
-  for (int kt = 0; kt < KT; ++kt) {
-    cp_async_wait<kStages - 3>();  // k-tile kt+1 landed
-    __syncthreads();               // ... for all threads; scale(kt) visible; compute(kt-1) finished everywhere
-    issue(kt + kStages - 1);       // refills the buffer compute(kt-1) just released
-    scale(kt + 1);
-    const double *as = As + ((kt % kStages) * kBM + wm + (lane >> 2)) * kLdK + (lane & 3);
-    const double *bs = Bs + ((kt % kStages) * kBM + wn + (lane >> 2)) * kLdK + (lane & 3);
-#pragma unroll
-    for (int kk = 0; kk < kBK / 4; ++kk) {
-      double a[8], b[4];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) a[i] = as[(8 * i) * kLdK + 4 * kk];
-#pragma unroll
-      for (int j = 0; j < 4; ++j) b[j] = bs[(8 * j) * kLdK + 4 * kk];
-#pragma unroll
-      for (int i = 0; i < 8; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) dmma_m8n8k4(acc[i][j], a[i], b[j]);
-    }
+    mbar_fence_init();
   }
-  cp_async_wait<0>();
+  __syncthreads();
 
-  double *Tz = Tpart + (int64_t)blockIdx.y * n_mo * n_mo;
-  const bool vec_ok = (n_mo & 1) == 0;
+  if (warp >= kConsumerWarps) {
+    // ------------------------------------------------ producers
+    reg_dec<88>();
+    const int pt = tid - kConsumerThreads, pw = pt >> 5;
+    const int c2 = (lane & 7) * 2;                // this thread's two columns of every k-tile
+    const int r0 = pw * 32 + (lane >> 3);         // its rows: r0 + 4j, j < 8
+    int nrowA = (n_mo - p0 - r0 + 3) >> 2, nrowB = (n_mo - q0 - r0 + 3) >> 2;   // valid rows among its 8
+    nrowA = max(0, min(8, nrowA));
+    nrowB = max(0, min(8, nrowB));
+    double eps_p[8];
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const int p = p0 + wm + 8 * i + (lane >> 2);
-    if (p < n_mo) {
+    for (int j = 0; j < 8; ++j) eps_p[j] = (j < nrowA) ? __ldg(eps + p0 + r0 + 4 * j) : 0.0;
+    const int64_t row_step = 4 * ldw;
+
+    // register prefetch of k-tile `kt`: the thread's 8 x 2 raw w values of the p rows, Omega of its two poles,
+    // eps_m and occ_m
+    double2 wv[8];
+    double om0, om1, em, fo;
+    int ld_m = m_begin, ld_ks = 0;
+    auto prefetch = [&](bool valid) {
+      if (valid) {
+        const int s = ld_ks * kBK + c2;
+        const int ncol = min(2, max(0, s_c - s));
+        const double *src = W + ((int64_t)ld_m * n_mo + p0 + r0) * ldw + s;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const int q = q0 + wn + 8 * j + 2 * (lane & 3);
-        if (q < n_mo) {
-          double *dst = Tz + (int64_t)p * n_mo + q;
-          if (vec_ok) {
-            double2 t = *reinterpret_cast<double2 *>(dst);
-            t.x += acc[i][j][0];
-            t.y += acc[i][j][1];
-            *reinterpret_cast<double2 *>(dst) = t;
-          } else {
-            dst[0] += acc[i][j][0];
-            if (q + 1 < n_mo) dst[1] += acc[i][j][1];
+        for (int j = 0; j < 8; ++j) {
+          double2 v = make_double2(0.0, 0.0);
+          if (j < nrowA && ncol > 0) {
+            v = __ldg(reinterpret_cast<const double2 *>(src + j * row_step));
+            if (ncol < 2) v.y = 0.0;
+          }
+          wv[j] = v;
+        }
+        om0 = __ldg(Omega + min(s, s_c - 1));
+        om1 = __ldg(Omega + min(s + 1, s_c - 1));
+        em = __ldg(eps + ld_m);
+        fo = __ldg(occ + ld_m);
+        if (++ld_ks == KTS) { ld_ks = 0; ++ld_m; }
+      }
+    };
+    prefetch(KT > 0);
+
+    int st = 0, cp_m = m_begin, cp_ks = 0;
+    uint32_t ph = 1;
+#pragma unroll 1
+    for (int kt = 0; kt < KT; ++kt) {
+      mbar_wait(empty + st, ph);
+      {  // q rows: raw copy
+        const int s = cp_ks * kBK + c2;
+        const int ncol = min(2, max(0, s_c - s));
+        const double *src = W + ((int64_t)cp_m * n_mo + q0 + r0) * ldw + s;
+        double *dst = Bs + (st * kBM + r0) * kLdK + c2;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int nb = (j < nrowB) ? ncol * 8 : 0;
+          cp_async_16(dst + 4 * j * kLdK, nb ? src + j * row_step : W, nb);
+        }
+        cp_async_mbar_arrive_noinc(full + st);
+        if (++cp_ks == KTS) { cp_ks = 0; ++cp_m; }
+      }
+      // p rows: take the prefetched registers, start the loads of the next k-tile, scale, store
+      double2 cur[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) cur[j] = wv[j];
+      const double c_om0 = om0, c_om1 = om1, c_em = em, c_fo = fo;
+      prefetch(kt + 1 < KT);
+      double *dstA = As + (st * kBM + r0) * kLdK + c2;
+      if (c_fo == 1.0) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const double d = eps_p[j] - c_em;
+          cur[j].x *= denominator_D<1>(d, c_om0, c_fo, eta2);
+          cur[j].y *= denominator_D<1>(d, c_om1, c_fo, eta2);
+        }
+      } else if (c_fo == 0.0) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const double d = eps_p[j] - c_em;
+          cur[j].x *= denominator_D<0>(d, c_om0, c_fo, eta2);
+          cur[j].y *= denominator_D<0>(d, c_om1, c_fo, eta2);
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const double d = eps_p[j] - c_em;
+          cur[j].x *= denominator_D<2>(d, c_om0, c_fo, eta2);
+          cur[j].y *= denominator_D<2>(d, c_om1, c_fo, eta2);
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) *reinterpret_cast<double2 *>(dstA + 4 * j * kLdK) = cur[j];
+      mbar_arrive(full + st);
+      if (++st == kSigmaStages) { st = 0; ph ^= 1; }
+    }
+    cp_async_wait_all();
+  } else {
+    // ------------------------------------------------ consumers
+    reg_inc<208>();
+    const FragMap fm(warp, lane, n_mo - p0, n_mo - q0);
+    const bool full_tile = fm.mi_cnt == 8 && fm.nj_cnt == 4;
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    int st = 0;
+    uint32_t ph = 0;
+#pragma unroll 1
+    for (int kt = 0; kt < KT; ++kt) {
+      mbar_wait(full + st, ph);
+      if (full_tile) mma_ktile_rowmajor<true>(acc, As + st * kBM * kLdK, Bs + st * kBM * kLdK, fm);
+      else mma_ktile_rowmajor<false>(acc, As + st * kBM * kLdK, Bs + st * kBM * kLdK, fm);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty + st);
+      if (++st == kSigmaStages) { st = 0; ph ^= 1; }
+    }
+
+    double *Tz = Tpart + (int64_t)blockIdx.y * n_mo * n_mo;
+    const bool vec_ok = (n_mo & 1) == 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int p = p0 + fm.row(i);
+      if (p < n_mo) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int q = q0 + fm.out_col(j);
+          if (q < n_mo) {
+            double *dst = Tz + (int64_t)p * n_mo + q;
+            if (vec_ok) {
+              double2 t = *reinterpret_cast<double2 *>(dst);
+              t.x += acc[i][j][0];
+              t.y += acc[i][j][1];
+              *reinterpret_cast<double2 *>(dst) = t;
+            } else {
+              dst[0] += acc[i][j][0];
+              if (q + 1 < n_mo) dst[1] += acc[i][j][1];
+            }
           }
         }
       }
