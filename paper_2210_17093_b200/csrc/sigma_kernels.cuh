@@ -83,9 +83,9 @@ constexpr size_t kSigmaSmemBytes = (size_t)kSigmaStages * 2 * kBM * kLdK * sizeo
 //   Omega [s_c]       excitation energies of the chunk
 //   Tpart [nsplit][N][N]  split-K partial tiles; slot z is owned by the CTAs with blockIdx.y == z and is
 //                     read-modify-written once per launch -> accumulation order is fixed, results reproducible.
-// Roles: the 4 producer warps form the operands -- the q rows of w go global -> shared by cp.async untouched, the
-// p rows go global -> registers (prefetched one k-tile ahead), are multiplied by D(m, s, eps_p) and stored to
-// shared: the scaled operand A = w.D exists only in shared memory.  The 8 consumer warps run LDS + DMMA only.
+// Roles: the 4 producer warps form the operands -- both row blocks of w go global -> shared by cp.async, two k-tiles
+// ahead; each producer thread then multiplies the chunks of the p rows it copied itself by D(m, s, eps_p) in
+// place: the scaled operand A = w.D exists only in shared memory.  The 8 consumer warps run LDS + DMMA only.
 __global__ void __launch_bounds__(kThreads, 1)
 sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double *__restrict__ eps,
                         const double *__restrict__ occ, const double *__restrict__ Omega, int n_mo, int s_c,
@@ -105,7 +105,7 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
 
   if (tid == 0) {
     for (int s = 0; s < kSigmaStages; ++s) {
-      mbar_init(full + s, 2 * kProducerThreads);   // per producer thread: one cp.async arrival (B tile) + one plain arrival (A tile)
+      mbar_init(full + s, kProducerThreads);
       mbar_init(empty + s, kConsumerWarps);
     }
     mbar_fence_init();
@@ -114,7 +114,7 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
 
   if (warp >= kConsumerWarps) {
     // ------------------------------------------------ producers
-    reg_dec<88>();
+    reg_dec<104>();
     const int pt = tid - kConsumerThreads, pw = pt >> 5;
     const int c2 = (lane & 7) * 2;                // this thread's two columns of every k-tile
     const int r0 = pw * 32 + (lane >> 3);         // its rows: r0 + 4j, j < 8
@@ -125,91 +125,79 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
 #pragma unroll
     for (int j = 0; j < 8; ++j) eps_p[j] = (j < nrowA) ? __ldg(eps + p0 + r0 + 4 * j) : 0.0;
     const int64_t row_step = 4 * ldw;
+    constexpr int kAhead = 2;                     // k-tiles whose cp.async are in flight ahead of the scaling
 
-    // register prefetch of k-tile `kt`: the thread's 8 x 2 raw w values of the p rows, Omega of its two poles,
-    // eps_m and occ_m
-    double2 wv[8];
-    double om0, om1, em, fo;
-    int ld_m = m_begin, ld_ks = 0;
-    auto prefetch = [&](bool valid) {
-      if (valid) {
+    // loader: raw w rows of both operands, global -> shared (cp.async); every thread later scales exactly the
+    // 16-byte chunks of the p rows it copied itself, so no producer-side barrier is needed
+    int ld_st = 0, ld_m = m_begin, ld_ks = 0;
+    uint32_t ld_ph = 1;                           // a fresh barrier passes a wait on parity 1
+    auto issue = [&](int kt) {
+      if (kt < KT) {
+        mbar_wait(empty + ld_st, ld_ph);
         const int s = ld_ks * kBK + c2;
         const int ncol = min(2, max(0, s_c - s));
-        const double *src = W + ((int64_t)ld_m * n_mo + p0 + r0) * ldw + s;
+        const double *srcA = W + ((int64_t)ld_m * n_mo + p0 + r0) * ldw + s;
+        const double *srcB = W + ((int64_t)ld_m * n_mo + q0 + r0) * ldw + s;
+        double *dstA = As + (ld_st * kBM + r0) * kLdK + c2;
+        double *dstB = Bs + (ld_st * kBM + r0) * kLdK + c2;
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-          double2 v = make_double2(0.0, 0.0);
-          if (j < nrowA && ncol > 0) {
-            v = __ldg(reinterpret_cast<const double2 *>(src + j * row_step));
-            if (ncol < 2) v.y = 0.0;
-          }
-          wv[j] = v;
+          const int nbA = (j < nrowA) ? ncol * 8 : 0, nbB = (j < nrowB) ? ncol * 8 : 0;
+          cp_async_16(dstA + 4 * j * kLdK, nbA ? srcA + j * row_step : W, nbA);
+          cp_async_16(dstB + 4 * j * kLdK, nbB ? srcB + j * row_step : W, nbB);
         }
-        om0 = __ldg(Omega + min(s, s_c - 1));
-        om1 = __ldg(Omega + min(s + 1, s_c - 1));
-        em = __ldg(eps + ld_m);
-        fo = __ldg(occ + ld_m);
         if (++ld_ks == KTS) { ld_ks = 0; ++ld_m; }
+        if (++ld_st == kSigmaStages) { ld_st = 0; ld_ph ^= 1; }
       }
+      cp_async_commit();
     };
-    prefetch(KT > 0);
+#pragma unroll
+    for (int i = 0; i < kAhead; ++i) issue(i);
 
-    int st = 0, cp_m = m_begin, cp_ks = 0;
-    uint32_t ph = 1;
+    int st = 0, sc_m = m_begin, sc_ks = 0;
 #pragma unroll 1
     for (int kt = 0; kt < KT; ++kt) {
-      mbar_wait(empty + st, ph);
-      {  // q rows: raw copy
-        const int s = cp_ks * kBK + c2;
-        const int ncol = min(2, max(0, s_c - s));
-        const double *src = W + ((int64_t)cp_m * n_mo + q0 + r0) * ldw + s;
-        double *dst = Bs + (st * kBM + r0) * kLdK + c2;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int nb = (j < nrowB) ? ncol * 8 : 0;
-          cp_async_16(dst + 4 * j * kLdK, nb ? src + j * row_step : W, nb);
-        }
-        cp_async_mbar_arrive_noinc(full + st);
-        if (++cp_ks == KTS) { cp_ks = 0; ++cp_m; }
-      }
-      // p rows: take the prefetched registers, start the loads of the next k-tile, scale, store
+      issue(kt + kAhead);
+      const int s = sc_ks * kBK + c2;
+      const double om0 = __ldg(Omega + min(s, s_c - 1)), om1 = __ldg(Omega + min(s + 1, s_c - 1));
+      const double em = __ldg(eps + sc_m), fo = __ldg(occ + sc_m);
+      cp_async_wait<kAhead>();                    // this thread's copies of k-tile kt have landed
+      double *rowA = As + (st * kBM + r0) * kLdK + c2;
       double2 cur[8];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) cur[j] = wv[j];
-      const double c_om0 = om0, c_om1 = om1, c_em = em, c_fo = fo;
-      prefetch(kt + 1 < KT);
-      double *dstA = As + (st * kBM + r0) * kLdK + c2;
-      if (c_fo == 1.0) {
+      for (int j = 0; j < 8; ++j) cur[j] = *reinterpret_cast<const double2 *>(rowA + 4 * j * kLdK);
+      if (fo == 1.0) {
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-          const double d = eps_p[j] - c_em;
-          cur[j].x *= denominator_D<1>(d, c_om0, c_fo, eta2);
-          cur[j].y *= denominator_D<1>(d, c_om1, c_fo, eta2);
+          const double d = eps_p[j] - em;
+          cur[j].x *= denominator_D<1>(d, om0, fo, eta2);
+          cur[j].y *= denominator_D<1>(d, om1, fo, eta2);
         }
-      } else if (c_fo == 0.0) {
+      } else if (fo == 0.0) {
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-          const double d = eps_p[j] - c_em;
-          cur[j].x *= denominator_D<0>(d, c_om0, c_fo, eta2);
-          cur[j].y *= denominator_D<0>(d, c_om1, c_fo, eta2);
+          const double d = eps_p[j] - em;
+          cur[j].x *= denominator_D<0>(d, om0, fo, eta2);
+          cur[j].y *= denominator_D<0>(d, om1, fo, eta2);
         }
       } else {
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-          const double d = eps_p[j] - c_em;
-          cur[j].x *= denominator_D<2>(d, c_om0, c_fo, eta2);
-          cur[j].y *= denominator_D<2>(d, c_om1, c_fo, eta2);
+          const double d = eps_p[j] - em;
+          cur[j].x *= denominator_D<2>(d, om0, fo, eta2);
+          cur[j].y *= denominator_D<2>(d, om1, fo, eta2);
         }
       }
 #pragma unroll
-      for (int j = 0; j < 8; ++j) *reinterpret_cast<double2 *>(dstA + 4 * j * kLdK) = cur[j];
-      mbar_arrive(full + st);
-      if (++st == kSigmaStages) { st = 0; ph ^= 1; }
+      for (int j = 0; j < 8; ++j) *reinterpret_cast<double2 *>(rowA + 4 * j * kLdK) = cur[j];
+      mbar_arrive(full + st);                     // release: the scaled p rows and the landed q rows of this thread
+      if (++sc_ks == KTS) { sc_ks = 0; ++sc_m; }
+      if (++st == kSigmaStages) st = 0;
     }
     cp_async_wait_all();
   } else {
     // ------------------------------------------------ consumers
-    reg_inc<208>();
+    reg_inc<200>();
     const FragMap fm(warp, lane, n_mo - p0, n_mo - q0);
     const bool full_tile = fm.mi_cnt == 8 && fm.nj_cnt == 4;
     double acc[8][4][2];
