@@ -10,6 +10,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <string>
 #include <vector>
@@ -195,7 +196,7 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
                                       (int)kSigmaSmemBytes));
     sigma_configured = true;
   }
-  const int nt = (p->n_mo + kBM - 1) / kBM;
+  const int ntp = (p->n_mo + kTP - 1) / kTP, ntq = (p->n_mo + kTQ - 1) / kTQ;
   for (int64_t v0 = 0; v0 < n_pole; v0 += p->v_cols) {
     const int64_t nv = std::min<int64_t>(p->v_cols, n_pole - v0);
     {  // stage 1 for all poles of this range at once (enough tiles to fill the SMs evenly):
@@ -218,8 +219,8 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
       }
       {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
         ScopedTimer t(p, kStage3);
-        sigma_accumulate_kernel<<<dim3(nt * nt, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
-            p->W, p->ldw, p->eps, p->occ, Omega + v0 + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, nt, p->Tpart);
+        sigma_accumulate_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
+            p->W, p->ldw, p->eps, p->occ, Omega + v0 + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart);
         p->kernel_launches += 1;
         QSGW_CUDA(p, cudaGetLastError());
       }
@@ -314,10 +315,10 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
     p->v_cols = std::min<int64_t>(round_up(n_pole_max, 2), cap);
   }
   p->ldv = round_up(p->v_cols, 2);
-  p->ldw = round_up(p->s_chunk, 2);
+  p->ldw = round_up(p->s_chunk, 2) + (getenv("QSGW_LDW_PAD") ? atoi(getenv("QSGW_LDW_PAD")) : 0);
   // split-K of stage 3 over the internal state m: enough CTAs for >= ~16 waves of the SMs, at most N splits
-  const int nt = (n_mo + kBM - 1) / kBM;
-  int want = (16 * prop.multiProcessorCount + nt * nt - 1) / (nt * nt);
+  const int nt2 = ((n_mo + kTP - 1) / kTP) * ((n_mo + kTQ - 1) / kTQ);
+  int want = (16 * prop.multiProcessorCount + nt2 - 1) / nt2;
   want = std::max(1, std::min(want, n_mo));
   p->m_per_split = (n_mo + want - 1) / want;
   p->nsplit = (n_mo + p->m_per_split - 1) / p->m_per_split;

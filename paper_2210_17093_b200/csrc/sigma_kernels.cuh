@@ -53,17 +53,17 @@ __global__ void pack_ov_transposed_kernel(const double *__restrict__ B, int n_mo
 // ---------------------------------------------------------------- stage 3
 // D(m,s,omega) = occ_m * x1/(x1^2+eta^2) + (1-occ_m) * x2/(x2^2+eta^2),  x1 = (omega-eps_m)+Omega_s,
 // x2 = (omega-eps_m)-Omega_s: real part of the two terms of Eq. (17).  d = omega - eps_m.
-// x/(x^2+eta^2) without the IEEE division's slow path: MUFU.RCP64H seed + two Newton steps folded into the
-// quotient (relative error ~2 ulp; x^2+eta^2 >= eta^2 > 0 is never subnormal for physical energies).
+// x/(x^2+eta^2) without the IEEE division's slow path: y = x^2+eta^2, r = MUFU.RCP64H(y) (relative error
+// e = 1 - y r, |e| <= 2^-20 measured), 1/y = r (1 + e + e^2 + O(e^3)), so x/y = q + q (e + e^2) with q = x r:
+// 5 FP64-pipe instructions, error <= 1 ulp (|e|^3 = 2^-60).  y >= eta^2 > 0 is never subnormal for physical energies.
 __device__ __forceinline__ double lehmann_term(double x, double eta2) {
   const double y = fma(x, x, eta2);
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
-  double e = fma(-y, r, 1.0);
-  r = fma(r, e, r);
   const double q = x * r;
-  e = fma(-y, r, 1.0);
-  return fma(q, e, q);
+  const double e = fma(-y, r, 1.0);
+  const double t = fma(e, e, e);
+  return fma(q, t, q);
 }
 
 // OCC: 1 = f_m == 1 (occupied), 0 = f_m == 0 (virtual), 2 = fractional (both terms)
@@ -74,10 +74,84 @@ __device__ __forceinline__ double denominator_D(double d, double Omega_s, double
   return occ_m * lehmann_term(d + Omega_s, eta2) + (1.0 - occ_m) * lehmann_term(d - Omega_s, eta2);
 }
 
+// Stage-3 CTA tile: 64 p rows x 256 q columns, k-tiles of 16 poles at one internal state m.  The tile is wide
+// in q because the D evaluations of a k-tile (one per element of the p operand) are amortised over the q width:
+// 64 x 16 evaluations against 64 x 256 x 16 FMA.  The 8 consumer warps are laid out 2 (p) x 4 (q), each owning
+// 4 x 8 DMMA fragments interleaved across the tile (p rows 16i + 8wmi + g, q columns 32j + 8wni + g), so ragged
+// edge tiles shed whole fragments evenly: granule 16 rows x 32 columns.
+constexpr int kTP = 64;
+constexpr int kTQ = 256;
 constexpr int kSigmaStages = 5;
-constexpr size_t kSigmaSmemBytes = (size_t)kSigmaStages * 2 * kBM * kLdK * sizeof(double) + 2 * kSigmaStages * sizeof(uint64_t);
+constexpr int kSigmaStageDoubles = (kTP + kTQ) * kBK;   // unpadded [row][16] tiles, XOR-swizzled (see sw_col)
+constexpr size_t kSigmaSmemBytes = (size_t)kSigmaStages * kSigmaStageDoubles * sizeof(double) + 2 * kSigmaStages * sizeof(uint64_t);
 
-// One CTA: output tile (tp, tq) of T, 128 x 128, for the internal states m in [z*m_per_split, ...) and all
+// Shared tiles of stage 3 are [row][16] doubles with the column index XOR-swizzled by 4 * (row & 3): a DMMA fragment
+// load (lanes g = 0..7 rows, t = 0..3 columns 4kk + t) then hits 16 distinct 8-byte bank pairs per half warp, and a
+// 16-byte cp.async chunk (2 columns) stays contiguous.  No padding: 5 stages of (64 + 256) x 16 doubles fit.
+__device__ __forceinline__ int sw_col(int row, int col) { return col ^ ((row & 3) << 2); }
+
+struct SigmaFragMap {
+  int wmi, wni, g, t;
+  int mi_cnt, nj_cnt;   // fragments of this warp with at least one valid row / column (warp-uniform)
+  __device__ __forceinline__ SigmaFragMap(int warp, int lane, int rows_valid, int cols_valid) {
+    wmi = warp & 1; wni = warp >> 1; g = lane >> 2; t = lane & 3;
+    const int rb = min(kTP / 8, (max(rows_valid, 0) + 7) >> 3), cb = min(kTQ / 8, (max(cols_valid, 0) + 7) >> 3);
+    mi_cnt = max(0, (rb - wmi + 1) >> 1);
+    nj_cnt = max(0, (cb - wni + 3) >> 2);
+  }
+  __device__ __forceinline__ int row(int i) const { return 16 * i + 8 * wmi + g; }
+  __device__ __forceinline__ int out_col(int j) const { return 32 * j + 8 * wni + 2 * t; }
+};
+
+// One k-tile of DMMA work: acc[i][j] += A[p rows of fragment i][k] * Wq[q rows of fragment j][k], k = 0..15, for the
+// first MI x NJ fragments of the warp.  MI, NJ are compile-time: a predicated-off DMMA still occupies the FP64 pipe
+// for its full issue time (measured: ncu counts it in sm__ops_path_tensor_src_fp64), so ragged edge tiles must
+// BRANCH around the fragments they do not own, not predicate them.
+template <int MI, int NJ>
+__device__ __forceinline__ void mma_ktile_sigma(double (&acc)[4][8][2], const double *ap, const double *bp, int gs) {
+#pragma unroll
+  for (int kk = 0; kk < kBK / 4; ++kk) {
+    const int off = (kk ^ gs) << 2;
+    double a[MI], b[NJ];
+#pragma unroll
+    for (int i = 0; i < MI; ++i) a[i] = ap[16 * i * kBK + off];
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) b[j] = bp[32 * j * kBK + off];
+#pragma unroll
+    for (int i = 0; i < MI; ++i)
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) dmma_m8n8k4(acc[i][j], a[i], b[j]);
+  }
+}
+
+template <int MI>
+__device__ __forceinline__ void mma_ktile_sigma_nj(double (&acc)[4][8][2], const double *ap, const double *bp, int gs, int nj) {
+  switch (nj) {
+    case 1: mma_ktile_sigma<MI, 1>(acc, ap, bp, gs); break;
+    case 2: mma_ktile_sigma<MI, 2>(acc, ap, bp, gs); break;
+    case 3: mma_ktile_sigma<MI, 3>(acc, ap, bp, gs); break;
+    case 4: mma_ktile_sigma<MI, 4>(acc, ap, bp, gs); break;
+    case 5: mma_ktile_sigma<MI, 5>(acc, ap, bp, gs); break;
+    case 6: mma_ktile_sigma<MI, 6>(acc, ap, bp, gs); break;
+    case 7: mma_ktile_sigma<MI, 7>(acc, ap, bp, gs); break;
+    case 8: mma_ktile_sigma<MI, 8>(acc, ap, bp, gs); break;
+    default: break;
+  }
+}
+
+// Ragged tile: dispatch (warp-uniform) on the fragment counts of this warp.
+__device__ __forceinline__ void mma_ktile_sigma_ragged(double (&acc)[4][8][2], const double *ap, const double *bp, int gs,
+                                                       int mi, int nj) {
+  switch (mi) {
+    case 1: mma_ktile_sigma_nj<1>(acc, ap, bp, gs, nj); break;
+    case 2: mma_ktile_sigma_nj<2>(acc, ap, bp, gs, nj); break;
+    case 3: mma_ktile_sigma_nj<3>(acc, ap, bp, gs, nj); break;
+    case 4: mma_ktile_sigma_nj<4>(acc, ap, bp, gs, nj); break;
+    default: break;
+  }
+}
+
+// One CTA: output tile (tp, tq) of T, 64 x 256, for the internal states m in [z*m_per_split, ...) and all
 // s_c poles of the chunk.  k-tiles of 16 poles at fixed m, so eps_m / occ_m are CTA-uniform per k-tile.
 //   W     [N*N][ldw]  chunk of residues, row m*N + p, column s (stage-2 output; both mirrors present)
 //   Omega [s_c]       excitation energies of the chunk
@@ -91,13 +165,12 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
                         const double *__restrict__ occ, const double *__restrict__ Omega, int n_mo, int s_c,
                         double eta2, int m_per_split, int ntq, double *__restrict__ Tpart) {
   extern __shared__ __align__(16) double smem[];
-  double *As = smem;                                  // [stage][128][kLdK]  p rows, already scaled by D
-  double *Bs = smem + kSigmaStages * kBM * kLdK;      // [stage][128][kLdK]  q rows, raw
-  uint64_t *full = reinterpret_cast<uint64_t *>(smem + 2 * kSigmaStages * kBM * kLdK);
+  // stage st: p rows at smem + st*kSigmaStageDoubles (already scaled by D when released), q rows kTP*kBK further
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + kSigmaStages * kSigmaStageDoubles);
   uint64_t *empty = full + kSigmaStages;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int tp = blockIdx.x / ntq, tq = blockIdx.x - tp * ntq;
-  const int p0 = tp * kBM, q0 = tq * kBN;
+  const int p0 = tp * kTP, q0 = tq * kTQ;
   const int m_begin = blockIdx.y * m_per_split;
   const int m_end = min(n_mo, m_begin + m_per_split);
   const int KTS = (s_c + kBK - 1) / kBK;         // k-tiles per m
@@ -114,16 +187,18 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
 
   if (warp >= kConsumerWarps) {
     // ------------------------------------------------ producers
-    reg_dec<104>();
+    reg_dec<72>();
     const int pt = tid - kConsumerThreads, pw = pt >> 5;
     const int c2 = (lane & 7) * 2;                // this thread's two columns of every k-tile
-    const int r0 = pw * 32 + (lane >> 3);         // its rows: r0 + 4j, j < 8
-    int nrowA = (n_mo - p0 - r0 + 3) >> 2, nrowB = (n_mo - q0 - r0 + 3) >> 2;   // valid rows among its 8
-    nrowA = max(0, min(8, nrowA));
-    nrowB = max(0, min(8, nrowB));
-    double eps_p[8];
+    const int rsub = lane >> 3;                   // rows rA0 + 4j (j < 4) of the p tile, rB0 + 4j (j < 16) of the q tile
+    const int rA0 = pw * (kTP / 4) + rsub, rB0 = pw * (kTQ / 4) + rsub;
+    const int nrowA = max(0, min(kTP / 16, (n_mo - p0 - rA0 + 3) >> 2));   // valid rows among its 4 / 16
+    const int nrowB = max(0, min(kTQ / 16, (n_mo - q0 - rB0 + 3) >> 2));
+    // all of a thread's rows are congruent to rsub mod 4, so one swizzled column offset serves them all
+    const int csw = sw_col(rsub, c2);
+    double eps_p[kTP / 16];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) eps_p[j] = (j < nrowA) ? __ldg(eps + p0 + r0 + 4 * j) : 0.0;
+    for (int j = 0; j < kTP / 16; ++j) eps_p[j] = (j < nrowA) ? __ldg(eps + p0 + rA0 + 4 * j) : 0.0;
     const int64_t row_step = 4 * ldw;
     constexpr int kAhead = 2;                     // k-tiles whose cp.async are in flight ahead of the scaling
 
@@ -136,15 +211,19 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
         mbar_wait(empty + ld_st, ld_ph);
         const int s = ld_ks * kBK + c2;
         const int ncol = min(2, max(0, s_c - s));
-        const double *srcA = W + ((int64_t)ld_m * n_mo + p0 + r0) * ldw + s;
-        const double *srcB = W + ((int64_t)ld_m * n_mo + q0 + r0) * ldw + s;
-        double *dstA = As + (ld_st * kBM + r0) * kLdK + c2;
-        double *dstB = Bs + (ld_st * kBM + r0) * kLdK + c2;
+        const double *srcA = W + ((int64_t)ld_m * n_mo + p0 + rA0) * ldw + s;
+        const double *srcB = W + ((int64_t)ld_m * n_mo + q0 + rB0) * ldw + s;
+        double *dstA = smem + ld_st * kSigmaStageDoubles + rA0 * kBK + csw;
+        double *dstB = smem + ld_st * kSigmaStageDoubles + (kTP + rB0) * kBK + csw;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int nbA = (j < nrowA) ? ncol * 8 : 0, nbB = (j < nrowB) ? ncol * 8 : 0;
-          cp_async_16(dstA + 4 * j * kLdK, nbA ? srcA + j * row_step : W, nbA);
-          cp_async_16(dstB + 4 * j * kLdK, nbB ? srcB + j * row_step : W, nbB);
+        for (int j = 0; j < kTP / 16; ++j) {
+          const int nb = (j < nrowA) ? ncol * 8 : 0;
+          cp_async_16(dstA + 4 * j * kBK, nb ? srcA + j * row_step : W, nb);
+        }
+#pragma unroll
+        for (int j = 0; j < kTQ / 16; ++j) {
+          const int nb = (j < nrowB) ? ncol * 8 : 0;
+          cp_async_16(dstB + 4 * j * kBK, nb ? srcB + j * row_step : W, nb);
         }
         if (++ld_ks == KTS) { ld_ks = 0; ++ld_m; }
         if (++ld_st == kSigmaStages) { ld_st = 0; ld_ph ^= 1; }
@@ -154,64 +233,71 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
 #pragma unroll
     for (int i = 0; i < kAhead; ++i) issue(i);
 
-    int st = 0, sc_m = m_begin, sc_ks = 0;
+    int st = 0, kt = 0;
 #pragma unroll 1
-    for (int kt = 0; kt < KT; ++kt) {
-      issue(kt + kAhead);
-      const int s = sc_ks * kBK + c2;
-      const double om0 = __ldg(Omega + min(s, s_c - 1)), om1 = __ldg(Omega + min(s + 1, s_c - 1));
-      const double em = __ldg(eps + sc_m), fo = __ldg(occ + sc_m);
-      cp_async_wait<kAhead>();                    // this thread's copies of k-tile kt have landed
-      double *rowA = As + (st * kBM + r0) * kLdK + c2;
-      double2 cur[8];
+    for (int m = m_begin; m < m_end; ++m) {
+      const double em = __ldg(eps + m), fo = __ldg(occ + m);
+      const long long fbits = __double_as_longlong(fo);
+      // occupation class by bit pattern (no FP64-pipe compare): 1.0 -> occupied term only, +-0.0 -> virtual term only
+      const int occ_class = (fbits == 0x3FF0000000000000LL) ? 1 : (((unsigned long long)fbits << 1) == 0ULL ? 0 : 2);
+      double d[kTP / 16];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) cur[j] = *reinterpret_cast<const double2 *>(rowA + 4 * j * kLdK);
-      if (fo == 1.0) {
+      for (int j = 0; j < kTP / 16; ++j) d[j] = eps_p[j] - em;
+#pragma unroll 1
+      for (int ks = 0; ks < KTS; ++ks, ++kt) {
+        issue(kt + kAhead);
+        const int s = ks * kBK + c2;
+        const double om0 = __ldg(Omega + min(s, s_c - 1)), om1 = __ldg(Omega + min(s + 1, s_c - 1));
+        cp_async_wait<kAhead>();                  // this thread's copies of k-tile kt have landed
+        double *rowA = smem + st * kSigmaStageDoubles + rA0 * kBK + csw;
+        double2 cur[kTP / 16];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const double d = eps_p[j] - em;
-          cur[j].x *= denominator_D<1>(d, om0, fo, eta2);
-          cur[j].y *= denominator_D<1>(d, om1, fo, eta2);
+        for (int j = 0; j < kTP / 16; ++j) cur[j] = *reinterpret_cast<const double2 *>(rowA + 4 * j * kBK);
+        if (occ_class == 1) {
+#pragma unroll
+          for (int j = 0; j < kTP / 16; ++j) {
+            cur[j].x *= denominator_D<1>(d[j], om0, fo, eta2);
+            cur[j].y *= denominator_D<1>(d[j], om1, fo, eta2);
+          }
+        } else if (occ_class == 0) {
+#pragma unroll
+          for (int j = 0; j < kTP / 16; ++j) {
+            cur[j].x *= denominator_D<0>(d[j], om0, fo, eta2);
+            cur[j].y *= denominator_D<0>(d[j], om1, fo, eta2);
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < kTP / 16; ++j) {
+            cur[j].x *= denominator_D<2>(d[j], om0, fo, eta2);
+            cur[j].y *= denominator_D<2>(d[j], om1, fo, eta2);
+          }
         }
-      } else if (fo == 0.0) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const double d = eps_p[j] - em;
-          cur[j].x *= denominator_D<0>(d, om0, fo, eta2);
-          cur[j].y *= denominator_D<0>(d, om1, fo, eta2);
-        }
-      } else {
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const double d = eps_p[j] - em;
-          cur[j].x *= denominator_D<2>(d, om0, fo, eta2);
-          cur[j].y *= denominator_D<2>(d, om1, fo, eta2);
-        }
+        for (int j = 0; j < kTP / 16; ++j) *reinterpret_cast<double2 *>(rowA + 4 * j * kBK) = cur[j];
+        mbar_arrive(full + st);                   // release: the scaled p rows and the landed q rows of this thread
+        if (++st == kSigmaStages) st = 0;
       }
-#pragma unroll
-      for (int j = 0; j < 8; ++j) *reinterpret_cast<double2 *>(rowA + 4 * j * kLdK) = cur[j];
-      mbar_arrive(full + st);                     // release: the scaled p rows and the landed q rows of this thread
-      if (++sc_ks == KTS) { sc_ks = 0; ++sc_m; }
-      if (++st == kSigmaStages) st = 0;
     }
     cp_async_wait_all();
   } else {
     // ------------------------------------------------ consumers
-    reg_inc<200>();
-    const FragMap fm(warp, lane, n_mo - p0, n_mo - q0);
-    const bool full_tile = fm.mi_cnt == 8 && fm.nj_cnt == 4;
-    double acc[8][4][2];
+    reg_inc<208>();
+    const SigmaFragMap fm(warp, lane, n_mo - p0, n_mo - q0);
+    const bool full_tile = fm.mi_cnt == 4 && fm.nj_cnt == 8;
+    double acc[4][8][2];
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < 4; ++i)
 #pragma unroll
-      for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+      for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
     int st = 0;
     uint32_t ph = 0;
 #pragma unroll 1
     for (int kt = 0; kt < KT; ++kt) {
       mbar_wait(full + st, ph);
-      if (full_tile) mma_ktile_rowmajor<true>(acc, As + st * kBM * kLdK, Bs + st * kBM * kLdK, fm);
-      else mma_ktile_rowmajor<false>(acc, As + st * kBM * kLdK, Bs + st * kBM * kLdK, fm);
+      const double *ap = smem + st * kSigmaStageDoubles + (8 * fm.wmi + fm.g) * kBK + fm.t;
+      const double *bp = smem + st * kSigmaStageDoubles + (kTP + 8 * fm.wni + fm.g) * kBK + fm.t;
+      if (full_tile) mma_ktile_sigma<4, 8>(acc, ap, bp, fm.g & 3);
+      else mma_ktile_sigma_ragged(acc, ap, bp, fm.g & 3, fm.mi_cnt, fm.nj_cnt);
       __syncwarp();
       if (lane == 0) mbar_arrive(empty + st);
       if (++st == kSigmaStages) { st = 0; ph ^= 1; }
@@ -220,11 +306,11 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
     double *Tz = Tpart + (int64_t)blockIdx.y * n_mo * n_mo;
     const bool vec_ok = (n_mo & 1) == 0;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
+    for (int i = 0; i < 4; ++i) {
       const int p = p0 + fm.row(i);
       if (p < n_mo) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < 8; ++j) {
           const int q = q0 + fm.out_col(j);
           if (q < n_mo) {
             double *dst = Tz + (int64_t)p * n_mo + q;
