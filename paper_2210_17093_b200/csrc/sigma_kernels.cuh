@@ -163,7 +163,7 @@ __device__ __forceinline__ void mma_ktile_sigma_ragged(double (&acc)[4][8][2], c
 __global__ void __launch_bounds__(kThreads, 1)
 sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double *__restrict__ eps,
                         const double *__restrict__ occ, const double *__restrict__ Omega, int n_mo, int s_c,
-                        double eta2, int m_per_split, int ntq, double *__restrict__ Tpart) {
+                        double eta2, int m_per_split, int ntq, double *__restrict__ Tpart, int dbg) {
   extern __shared__ __align__(16) double smem[];
   // stage st: p rows at smem + st*kSigmaStageDoubles (already scaled by D when released), q rows kTP*kBK further
   uint64_t *full = reinterpret_cast<uint64_t *>(smem + kSigmaStages * kSigmaStageDoubles);
@@ -253,7 +253,8 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
         double2 cur[kTP / 16];
 #pragma unroll
         for (int j = 0; j < kTP / 16; ++j) cur[j] = *reinterpret_cast<const double2 *>(rowA + 4 * j * kBK);
-        if (occ_class == 1) {
+        if (dbg == 1) {
+        } else if (occ_class == 1) {
 #pragma unroll
           for (int j = 0; j < kTP / 16; ++j) {
             cur[j].x *= denominator_D<1>(d[j], om0, fo, eta2);
