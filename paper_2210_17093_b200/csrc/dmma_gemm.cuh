@@ -25,7 +25,8 @@ constexpr int kBN = 128;
 constexpr int kBK = 16;
 constexpr int kLdT = kBM + 4;   // k-major tile rows [k][128 + 4]: ld = 4 (mod 16) doubles -> LDS.64 fragments conflict-free
 constexpr int kLdK = kBK + 4;   // row-major tile rows [row][16 + 4]: same property for the [row][k] layout of stage 3
-constexpr int kGemmStages = 6;
+constexpr int kGBK = 32;          // k depth of one ring stage of the stage-1/2 GEMM (two barrier round trips per 8 k4 steps cost ~2 %)
+constexpr int kGemmStages = 3;
 
 // D(2 regs) += A(8x4, row) * B(4x8, col); lane holds A[lane/4][lane%4], B[lane%4][lane/4],
 // D[lane/4][2*(lane%4) + {0,1}].
@@ -44,6 +45,12 @@ __device__ __forceinline__ void cp_async_16(void *smem_dst, const void *gmem_src
 __device__ __forceinline__ void cp_async_8(void *smem_dst, const void *gmem_src, int src_bytes) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(src_bytes)
                : "memory");
+}
+__device__ __forceinline__ void cp_async_16_s(uint32_t smem_dst, const void *gmem_src, int src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_dst), "l"(gmem_src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_8_s(uint32_t smem_dst, const void *gmem_src, int src_bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_dst), "l"(gmem_src), "r"(src_bytes) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -97,13 +104,13 @@ struct FragMap {
   __device__ __forceinline__ int out_col(int j) const { return 32 * j + 8 * wni + 2 * t; }  // first of this lane's 2 accumulator columns
 };
 
-// One k-tile (16 deep) of DMMA work on k-major tiles As[k][kLdT], Bs[k][kLdT].
+// One k-tile (kGBK deep) of DMMA work on k-major tiles As[k][kLdT], Bs[k][kLdT].
 template <bool FULL>
 __device__ __forceinline__ void mma_ktile_kmajor(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
   const double *ap = as + 8 * fm.wmi + fm.g + fm.t * kLdT;
   const double *bp = bs + 8 * fm.wni + fm.g + fm.t * kLdT;
 #pragma unroll
-  for (int kk = 0; kk < kBK / 4; ++kk) {
+  for (int kk = 0; kk < kGBK / 4; ++kk) {
     double a[8], b[4];
 #pragma unroll
     for (int i = 0; i < 8; ++i)
@@ -118,6 +125,46 @@ __device__ __forceinline__ void mma_ktile_kmajor(double (&acc)[8][4][2], const d
         for (int j = 0; j < 4; ++j)
           if (FULL || j < fm.nj_cnt) dmma_m8n8k4(acc[i][j], a[i], b[j]);
       }
+  }
+}
+
+// Ragged in M only (the last row of tiles of stage 1 / stage 2): the first MI row fragments, all 4 column fragments,
+// with MI a compile-time constant -- a predicated-off DMMA still costs its pipe time, so the fragments a warp does not
+// own must be branched around, not predicated.
+template <int MI>
+__device__ __forceinline__ void mma_ktile_kmajor_rows(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
+  const double *ap = as + 8 * fm.wmi + fm.g + fm.t * kLdT;
+  const double *bp = bs + 8 * fm.wni + fm.g + fm.t * kLdT;
+#pragma unroll
+  for (int kk = 0; kk < kGBK / 4; ++kk) {
+    double a[MI], b[4];
+#pragma unroll
+    for (int i = 0; i < MI; ++i) a[i] = ap[kk * 4 * kLdT + 16 * i];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) b[j] = bp[kk * 4 * kLdT + 32 * j];
+#pragma unroll
+    for (int i = 0; i < MI; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) dmma_m8n8k4(acc[i][j], a[i], b[j]);
+  }
+}
+
+// Dispatch of one k-tile on the (warp-uniform) fragment counts of the tile.
+__device__ __forceinline__ void mma_ktile_kmajor_any(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
+  if (fm.nj_cnt == 4) {
+    switch (fm.mi_cnt) {
+      case 8: mma_ktile_kmajor_rows<8>(acc, as, bs, fm); break;
+      case 7: mma_ktile_kmajor_rows<7>(acc, as, bs, fm); break;
+      case 6: mma_ktile_kmajor_rows<6>(acc, as, bs, fm); break;
+      case 5: mma_ktile_kmajor_rows<5>(acc, as, bs, fm); break;
+      case 4: mma_ktile_kmajor_rows<4>(acc, as, bs, fm); break;
+      case 3: mma_ktile_kmajor_rows<3>(acc, as, bs, fm); break;
+      case 2: mma_ktile_kmajor_rows<2>(acc, as, bs, fm); break;
+      case 1: mma_ktile_kmajor_rows<1>(acc, as, bs, fm); break;
+      default: break;
+    }
+  } else {
+    mma_ktile_kmajor<false>(acc, as, bs, fm);   // ragged in N too (last tile column of the last chunk): rare
   }
 }
 
@@ -145,32 +192,39 @@ __device__ __forceinline__ void mma_ktile_rowmajor(double (&acc)[8][4][2], const
   }
 }
 
-// Producer side: stage one k-major operand tile dst[k][c] = src[k*ld + c], k < kBK, c < 128, with the 128 producer
+// Producer side: stage one k-major operand tile dst[k][c] = src[k*ld + c], k < kGBK, c < 128, with the 128 producer
 // threads (pt = 0..127); rows >= kvalid and columns >= cvalid are zero-filled.  VEC = doubles per cp.async
 // (2 needs 16-byte aligned src rows).
 template <int VEC>
 __device__ __forceinline__ void load_tile_kmajor(double *dst, const double *src, int64_t ld, int kvalid, int cvalid,
                                                  const double *safe, int pt) {
+  // running source pointer / 32-bit shared address: few live registers, so the 40-72 register producers do not spill
   if (VEC == 2) {
     const int c = (pt & 63) * 2, r0 = pt >> 6;
     int n = cvalid - c;
     n = n < 0 ? 0 : (n > 2 ? 2 : n);
+    const int nbytes = n * 8;
     const double *s = src + (int64_t)r0 * ld + c;
-    double *d = dst + r0 * kLdT + c;
-#pragma unroll
-    for (int j = 0; j < kBK / 2; ++j) {
-      const int nb = (r0 + 2 * j < kvalid) ? n * 8 : 0;
-      cp_async_16(d + 2 * j * kLdT, nb ? s + (int64_t)(2 * j) * ld : safe, nb);
+    uint32_t d = smem_u32(dst + r0 * kLdT + c);
+    const int64_t step = 2 * ld;
+#pragma unroll 4
+    for (int j = 0; j < kGBK / 2; ++j) {
+      const int nb = (r0 + 2 * j < kvalid) ? nbytes : 0;
+      cp_async_16_s(d, nb ? s : safe, nb);
+      s += step;
+      d += 2 * kLdT * (int)sizeof(double);
     }
   } else {
     const int c = pt;
     const int nbc = (c < cvalid) ? 8 : 0;
     const double *s = src + c;
-    double *d = dst + c;
-#pragma unroll
-    for (int r = 0; r < kBK; ++r) {
+    uint32_t d = smem_u32(dst + c);
+#pragma unroll 4
+    for (int r = 0; r < kGBK; ++r) {
       const int nb = (r < kvalid) ? nbc : 0;
-      cp_async_8(d + r * kLdT, nb ? s + (int64_t)r * ld : safe, nb);
+      cp_async_8_s(d, nb ? s : safe, nb);
+      s += ld;
+      d += kLdT * (int)sizeof(double);
     }
   }
 }
@@ -181,7 +235,9 @@ struct EpiStore {
   double *C;
   int64_t ldc;
   double alpha;
-  __device__ __forceinline__ void operator()(int row, int col, double v0, double v1, int ncols) const {
+  using RowCtx = int;
+  __device__ __forceinline__ RowCtx row_ctx(int) const { return 0; }
+  __device__ __forceinline__ void operator()(RowCtx, int row, int col, double v0, double v1, int ncols) const {
     double *dst = C + (int64_t)row * ldc + col;
     if (col + 1 < ncols && ((ldc & 1) == 0)) {
       *reinterpret_cast<double2 *>(dst) = make_double2(alpha * v0, alpha * v1);
@@ -200,8 +256,9 @@ struct EpiPairScatter {
   const int2 *pairs;
   int n_mo;
   double alpha;
-  __device__ __forceinline__ void operator()(int row, int col, double v0, double v1, int ncols) const {
-    const int2 pm = __ldg(pairs + row);
+  using RowCtx = int2;
+  __device__ __forceinline__ RowCtx row_ctx(int row) const { return __ldg(pairs + row); }
+  __device__ __forceinline__ void operator()(RowCtx pm, int, int col, double v0, double v1, int ncols) const {
     double *d0 = W + ((int64_t)pm.y * n_mo + pm.x) * ldw + col;
     double *d1 = W + ((int64_t)pm.x * n_mo + pm.y) * ldw + col;
     v0 *= alpha;
@@ -216,27 +273,24 @@ struct EpiPairScatter {
   }
 };
 
-constexpr size_t kGemmSmemBytes = (size_t)kGemmStages * 2 * kBK * kLdT * sizeof(double) + 2 * kGemmStages * sizeof(uint64_t);
+constexpr size_t kGemmSmemBytes = (size_t)kGemmStages * 2 * kGBK * kLdT * sizeof(double) + 2 * kGemmStages * sizeof(uint64_t);
 
 // C(M x N) = epilogue( sum_k A[k][m] * B[k][n] ),  A stored [K][lda] (m contiguous), B stored [K][ldb] (n contiguous).
 // A must be 16-byte aligned with even lda (library workspace); B may be arbitrary when VECB == 1.
-// grid.x = ntm * ntn tiles of 128 x 128; m_fastest picks which tile index varies fastest (the dimension with fewer
-// tiles, so that concurrently running CTAs share operand panels in L2).
+// ntm * ntn tiles of 128 x 128 dealt round-robin to the grid; m_fastest picks which tile index varies fastest (the
+// dimension with fewer tiles, so that concurrently running CTAs share operand panels in L2).
 template <int VECB, class Epi>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_tn_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__restrict__ Bm, int64_t ldb, int M, int N,
                     int K, int ntm, int ntn, int m_fastest, Epi epi) {
   extern __shared__ __align__(16) double smem[];
   double *As = smem;
-  double *Bs = smem + kGemmStages * kBK * kLdT;
-  uint64_t *full = reinterpret_cast<uint64_t *>(smem + 2 * kGemmStages * kBK * kLdT);
+  double *Bs = smem + kGemmStages * kGBK * kLdT;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + 2 * kGemmStages * kGBK * kLdT);
   uint64_t *empty = full + kGemmStages;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  int tm, tn;
-  if (m_fastest) { tn = blockIdx.x / ntm; tm = blockIdx.x - tn * ntm; }
-  else { tm = blockIdx.x / ntn; tn = blockIdx.x - tm * ntn; }
-  const int m0 = tm * kBM, n0 = tn * kBN;
-  const int KT = (K + kBK - 1) / kBK;
+  const int KT = (K + kGBK - 1) / kGBK;
+  const int ntiles = ntm * ntn;
 
   if (tid == 0) {
     for (int s = 0; s < kGemmStages; ++s) {
@@ -247,50 +301,69 @@ gemm_tn_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__r
   }
   __syncthreads();
 
+  // Tiles blockIdx.x, blockIdx.x + gridDim.x, ...: with gridDim.x = ntiles this is one tile per CTA; with one CTA per
+  // SM it is a persistent kernel whose operand ring runs on across tile boundaries, so the producers prefetch the
+  // next tile's first k-tiles while the consumers store the current tile.
   if (warp >= kConsumerWarps) {
     // ------------------------------------------------ producers: cp.async the k-tiles into the ring
     reg_dec<40>();
     const int pt = tid - kConsumerThreads;
     int st = 0;
     uint32_t ph = 1;   // a fresh barrier passes a wait on parity 1: the first pass over the ring does not block
-    for (int kt = 0; kt < KT; ++kt) {
-      mbar_wait(empty + st, ph);
-      const int k0 = kt * kBK;
-      load_tile_kmajor<2>(As + st * kBK * kLdT, A + (int64_t)k0 * lda + m0, lda, K - k0, M - m0, A, pt);
-      load_tile_kmajor<VECB>(Bs + st * kBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, K - k0, N - n0, Bm, pt);
-      cp_async_mbar_arrive_noinc(full + st);
-      if (++st == kGemmStages) { st = 0; ph ^= 1; }
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      int tm, tn;
+      if (m_fastest) { tn = tile / ntm; tm = tile - tn * ntm; }
+      else { tm = tile / ntn; tn = tile - tm * ntn; }
+      const int m0 = tm * kBM, n0 = tn * kBN;
+      for (int kt = 0; kt < KT; ++kt) {
+        mbar_wait(empty + st, ph);
+        const int k0 = kt * kGBK;
+        load_tile_kmajor<2>(As + st * kGBK * kLdT, A + (int64_t)k0 * lda + m0, lda, K - k0, M - m0, A, pt);
+        load_tile_kmajor<VECB>(Bs + st * kGBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, K - k0, N - n0, Bm, pt);
+        cp_async_mbar_arrive_noinc(full + st);
+        if (++st == kGemmStages) { st = 0; ph ^= 1; }
+      }
     }
     cp_async_wait_all();
   } else {
     // ------------------------------------------------ consumers: LDS.64 fragments + DMMA
     reg_inc<232>();
-    const FragMap fm(warp, lane, M - m0, N - n0);
-    const bool full_tile = fm.mi_cnt == 8 && fm.nj_cnt == 4;
-    double acc[8][4][2];
-#pragma unroll
-    for (int i = 0; i < 8; ++i)
-#pragma unroll
-      for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
     int st = 0;
     uint32_t ph = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      int tm, tn;
+      if (m_fastest) { tn = tile / ntm; tm = tile - tn * ntm; }
+      else { tm = tile / ntn; tn = tile - tm * ntn; }
+      const int m0 = tm * kBM, n0 = tn * kBN;
+      const FragMap fm(warp, lane, M - m0, N - n0);
+      const bool full_tile = fm.mi_cnt == 8 && fm.nj_cnt == 4;
+      // per-row epilogue context (stage 2: the (p, m) pair of the row), fetched now so its latency hides behind the k loop
+      typename Epi::RowCtx rc[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) rc[i] = epi.row_ctx(min(m0 + fm.row(i), M - 1));
+      double acc[8][4][2];
+#pragma unroll
+      for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 #pragma unroll 1
-    for (int kt = 0; kt < KT; ++kt) {
-      mbar_wait(full + st, ph);
-      if (full_tile) mma_ktile_kmajor<true>(acc, As + st * kBK * kLdT, Bs + st * kBK * kLdT, fm);
-      else mma_ktile_kmajor<false>(acc, As + st * kBK * kLdT, Bs + st * kBK * kLdT, fm);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(empty + st);
-      if (++st == kGemmStages) { st = 0; ph ^= 1; }
-    }
+      for (int kt = 0; kt < KT; ++kt) {
+        mbar_wait(full + st, ph);
+        if (full_tile) mma_ktile_kmajor_rows<8>(acc, As + st * kGBK * kLdT, Bs + st * kGBK * kLdT, fm);
+        else mma_ktile_kmajor_any(acc, As + st * kGBK * kLdT, Bs + st * kGBK * kLdT, fm);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty + st);
+        if (++st == kGemmStages) { st = 0; ph ^= 1; }
+      }
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const int row = m0 + fm.row(i);
-      if (row < M) {
+      for (int i = 0; i < 8; ++i) {
+        const int row = m0 + fm.row(i);
+        if (row < M) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int col = n0 + fm.out_col(j);
-          if (col < N) epi(row, col, acc[i][j][0], acc[i][j][1], N);
+          for (int j = 0; j < 4; ++j) {
+            const int col = n0 + fm.out_col(j);
+            if (col < N) epi(rc[i], row, col, acc[i][j][0], acc[i][j][1], N);
+          }
         }
       }
     }

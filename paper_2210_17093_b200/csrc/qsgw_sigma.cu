@@ -38,7 +38,7 @@ struct qsgw_sigma_plan {
   int s_chunk = 0;
   int64_t v_cols = 0;   // poles per stage-1 launch (V holds this many columns)
   cudaStream_t stream = nullptr;
-  int device = 0;
+  int device = 0, num_sms = 0;
 
   // workspace
   int64_t n_pair = 0, ldp = 0, ld_aux = 0, ldv = 0, ldw = 0;
@@ -150,7 +150,8 @@ int launch_gemm(qsgw_sigma_plan *p, const double *A, int64_t lda, const double *
   const int ntm = (M + kBM - 1) / kBM, ntn = (N + kBN - 1) / kBN;
   if ((int64_t)ntm * ntn > INT32_MAX) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "GEMM grid too large");
   // the dimension with fewer tiles varies fastest: the CTAs of one wave then share its few operand panels in L2
-  kern<<<ntm * ntn, kThreads, kGemmSmemBytes, p->stream>>>(A, lda, Bm, ldb, M, N, K, ntm, ntn, ntm <= ntn ? 1 : 0, epi);
+  // persistent: one CTA per SM walks the tiles round-robin
+  kern<<<std::min(ntm * ntn, p->num_sms), kThreads, kGemmSmemBytes, p->stream>>>(A, lda, Bm, ldb, M, N, K, ntm, ntn, ntm <= ntn ? 1 : 0, epi);
   p->kernel_launches += 1;
   QSGW_CUDA(p, cudaGetLastError());
   return QSGW_SIGMA_OK;
@@ -300,6 +301,7 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
   qsgw_sigma_plan *p = new (std::nothrow) qsgw_sigma_plan;
   if (!p) return fail(nullptr, QSGW_SIGMA_ERR_ALLOC, "create: out of host memory");
   p->device = dev;
+  p->num_sms = prop.multiProcessorCount;
   p->n_mo = n_mo; p->n_occ = n_occ; p->n_virt = n_mo - n_occ; p->n_aux = n_aux;
   p->n_ov = (int64_t)n_occ * p->n_virt;
   p->n_pole_max = n_pole_max;
@@ -315,7 +317,7 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
     p->v_cols = std::min<int64_t>(round_up(n_pole_max, 2), cap);
   }
   p->ldv = round_up(p->v_cols, 2);
-  p->ldw = round_up(p->s_chunk, 2) + (getenv("QSGW_LDW_PAD") ? atoi(getenv("QSGW_LDW_PAD")) : 0);
+  p->ldw = round_up(p->s_chunk, 2);
   // split-K of stage 3 over the internal state m: enough CTAs for >= ~16 waves of the SMs, at most N splits
   const int nt2 = ((n_mo + kTP - 1) / kTP) * ((n_mo + kTQ - 1) / kTQ);
   int want = (16 * prop.multiProcessorCount + nt2 - 1) / nt2;
