@@ -221,7 +221,7 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
       {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
         ScopedTimer t(p, kStage3);
         sigma_accumulate_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
-            p->W, p->ldw, p->eps, p->occ, Omega + v0 + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart, getenv("QSGW_DBG") ? atoi(getenv("QSGW_DBG")) : 0);
+            p->W, p->ldw, p->eps, p->occ, Omega + v0 + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart);
         p->kernel_launches += 1;
         QSGW_CUDA(p, cudaGetLastError());
       }

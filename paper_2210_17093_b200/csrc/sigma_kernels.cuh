@@ -163,7 +163,7 @@ __device__ __forceinline__ void mma_ktile_sigma_ragged(double (&acc)[4][8][2], c
 __global__ void __launch_bounds__(kThreads, 1)
 sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double *__restrict__ eps,
                         const double *__restrict__ occ, const double *__restrict__ Omega, int n_mo, int s_c,
-                        double eta2, int m_per_split, int ntq, double *__restrict__ Tpart, int dbg) {
+                        double eta2, int m_per_split, int ntq, double *__restrict__ Tpart) {
   extern __shared__ __align__(16) double smem[];
   // stage st: p rows at smem + st*kSigmaStageDoubles (already scaled by D when released), q rows kTP*kBK further
   uint64_t *full = reinterpret_cast<uint64_t *>(smem + kSigmaStages * kSigmaStageDoubles);
@@ -187,7 +187,7 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
 
   if (warp >= kConsumerWarps) {
     // ------------------------------------------------ producers
-    reg_dec<72>();
+    reg_dec<136>();
     const int pt = tid - kConsumerThreads, pw = pt >> 5;
     const int c2 = (lane & 7) * 2;                // this thread's two columns of every k-tile
     const int rsub = lane >> 3;                   // rows rA0 + 4j (j < 4) of the p tile, rB0 + 4j (j < 16) of the q tile
@@ -240,6 +240,7 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
       const long long fbits = __double_as_longlong(fo);
       // occupation class by bit pattern (no FP64-pipe compare): 1.0 -> occupied term only, +-0.0 -> virtual term only
       const int occ_class = (fbits == 0x3FF0000000000000LL) ? 1 : (((unsigned long long)fbits << 1) == 0ULL ? 0 : 2);
+      const double sgn = occ_class == 1 ? 1.0 : -1.0;
       double d[kTP / 16];
 #pragma unroll
       for (int j = 0; j < kTP / 16; ++j) d[j] = eps_p[j] - em;
@@ -253,18 +254,30 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
         double2 cur[kTP / 16];
 #pragma unroll
         for (int j = 0; j < kTP / 16; ++j) cur[j] = *reinterpret_cast<const double2 *>(rowA + 4 * j * kBK);
-        if (dbg == 1) {
-        } else if (occ_class == 1) {
+        if (occ_class != 2) {
+          // f_m in {0, 1}: one Lehmann term, x = d + sgn * Omega_s.  The 8 evaluations advance together, stage by
+          // stage, so that each dependent step is ONE burst of 8 independent FP64 instructions: the producer warp
+          // shares its sub-partition's FP64 pipe with two DMMA streams and pays an arbitration wait per burst.
+          constexpr int E = kTP / 8;
+          double x[E], y[E], r[E];
+#pragma unroll
+          for (int e = 0; e < E; ++e) x[e] = fma(sgn, (e & 1) ? om1 : om0, d[e >> 1]);
+#pragma unroll
+          for (int e = 0; e < E; ++e) y[e] = fma(x[e], x[e], eta2);
+#pragma unroll
+          for (int e = 0; e < E; ++e) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r[e]) : "d"(y[e]));
+#pragma unroll
+          for (int e = 0; e < E; ++e) x[e] *= r[e];                      // q = x r
+#pragma unroll
+          for (int e = 0; e < E; ++e) y[e] = fma(-y[e], r[e], 1.0);      // e = 1 - y r
+#pragma unroll
+          for (int e = 0; e < E; ++e) y[e] = fma(y[e], y[e], y[e]);      // t = e + e^2
+#pragma unroll
+          for (int e = 0; e < E; ++e) x[e] = fma(x[e], y[e], x[e]);      // D = q + q t
 #pragma unroll
           for (int j = 0; j < kTP / 16; ++j) {
-            cur[j].x *= denominator_D<1>(d[j], om0, fo, eta2);
-            cur[j].y *= denominator_D<1>(d[j], om1, fo, eta2);
-          }
-        } else if (occ_class == 0) {
-#pragma unroll
-          for (int j = 0; j < kTP / 16; ++j) {
-            cur[j].x *= denominator_D<0>(d[j], om0, fo, eta2);
-            cur[j].y *= denominator_D<0>(d[j], om1, fo, eta2);
+            cur[j].x *= x[2 * j];
+            cur[j].y *= x[2 * j + 1];
           }
         } else {
 #pragma unroll
@@ -282,7 +295,7 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
     cp_async_wait_all();
   } else {
     // ------------------------------------------------ consumers
-    reg_inc<208>();
+    reg_inc<184>();
     const SigmaFragMap fm(warp, lane, n_mo - p0, n_mo - q0);
     const bool full_tile = fm.mi_cnt == 4 && fm.nj_cnt == 8;
     double acc[4][8][2];
