@@ -32,6 +32,8 @@ METRIC = "sigma_c_build_fp64_tflops"
 UNIT = "TFLOP/s"
 # FP64 pipe of sm_100a: DMMA.8x8x4 and DFMA both retire 64 FMA/clk/SM (measured: profiles/r01_fp64_peaks.md)
 FP64_FMA_PER_CLK_PER_SM = 64
+# dram__bytes_read.sum + dram__bytes_write.sum of one stage-2 launch over a full s-block (profiles/r01_full_large.md)
+NCU_STAGE2_DRAM_BYTES_PER_LAUNCH = {"large": 37.488597e9 + 11.782985e9}
 
 
 def _peaks():
@@ -264,7 +266,8 @@ def run_gpu(args):
             "tflops_model_full": world * fl["F_full"] / (ms_per_step * 1e-3) / 1e12,
             "frac_of_fp64_peak": value / (world * peak),
             "fp64_peak_tflops": {"value": peak, "how": f"{nsm} SMs x {FP64_FMA_PER_CLK_PER_SM} FMA/clk x 2 x sm_max_mhz of MEASURED_PEAKS.json ({peak_src})",
-                                 "dmma_microbench": 36.98, "cublas_dgemm_8192": 35.47,
+                                 "dmma_microbench": 36.74, "lds_fed_dmma_microbench": 37.01, "cublas_dgemm_8192": 35.44,
+                                 "source": "profiles/r01_fp64_peaks.md",
                                  "bf16_measured_x_nominal_ratio": bf16_ratio_peak},
             "stage_ms_per_build": {k[3:]: stats[k] / args.steps for k in ("ms_pack", "ms_stage1", "ms_stage2", "ms_stage3", "ms_epilogue")},
             "stage_tflops": {"stage1": fl["F1"] * args.steps / max(stats["ms_stage1"], 1e-9) / 1e9,
@@ -272,7 +275,8 @@ def run_gpu(args):
                              "stage3": fl["F3"] * args.steps / max(stats["ms_stage3"], 1e-9) / 1e9},
             "roofline": {"bound": "tensor", "kernel": "gemm_tn_dmma_kernel<2,EpiPairScatter> (stage 2, w producer)",
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "launches": stats["launches_stage2"], "avg_launch_ms": s2_ms, "traffic": None,
+                         "launches": stats["launches_stage2"], "avg_launch_ms": s2_ms,
+                         "traffic": NCU_STAGE2_DRAM_BYTES_PER_LAUNCH.get(cfg.name), "traffic_unit": "bytes per launch (dram read + write, ncu --set full, profiles/r01_full_large.md)",
                          "peak_source": f"FP64 pipe rate at max SM clock ({peak_src} MEASURED_PEAKS.json sm_max_mhz); no FP64 entry is measured there"},
             "gpu_launches": stats["kernel_launches"],
             "wall_s_timed_region": t_wall,

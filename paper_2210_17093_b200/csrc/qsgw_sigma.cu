@@ -318,9 +318,9 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
   }
   p->ldv = round_up(p->v_cols, 2);
   p->ldw = round_up(p->s_chunk, 2);
-  // split-K of stage 3 over the internal state m: enough CTAs for >= ~16 waves of the SMs, at most N splits
+  // split-K of stage 3 over the internal state m: enough CTAs for ~40 waves of the SMs (ragged edge tiles run 2-3x shorter than full ones: the tail of a launch is one CTA long), at most N splits
   const int nt2 = ((n_mo + kTP - 1) / kTP) * ((n_mo + kTQ - 1) / kTQ);
-  int want = (16 * prop.multiProcessorCount + nt2 - 1) / nt2;
+  int want = (40 * prop.multiProcessorCount + nt2 - 1) / nt2;
   want = std::max(1, std::min(want, n_mo));
   p->m_per_split = (n_mo + want - 1) / want;
   p->nsplit = (n_mo + p->m_per_split - 1) / p->m_per_split;
