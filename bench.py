@@ -162,6 +162,22 @@ def _config_dict(cfg, args, extra=None):
     return d
 
 
+def max_over_ranks(ms: float, world: int, device="cpu") -> float:
+    """Replicas only: the one data-free collective of the bench -- the max over ranks of a rank-local time."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(flops_per_rank: float, world: int, ms_per_step: float) -> float:
+    """Weak scaling: every rank builds its own Sigma, so the job's TFLOP/s is world x flops over the slowest rank's time."""
+    return world * flops_per_rank / (ms_per_step * 1e-3) / 1e12
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -241,13 +257,10 @@ def run_gpu(args):
         t_wall = time.perf_counter() - t_wall0
     step_ms = [sum(a.elapsed_time(b) for a, b in evs) for evs in all_events]
     total_ms = sum(step_ms)
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, dev)
     stats = pkg.qsgw_sigma_get_stats(plan, reset=True)
     ms_per_step = total_ms / args.steps
-    value = world * fl["F_min"] / (ms_per_step * 1e-3) / 1e12
+    value = whole_job_value(fl["F_min"], world, ms_per_step)
     assert torch.isfinite(Sigma).all()
 
     out = None
@@ -301,13 +314,9 @@ def run_gpu(args):
         e1.record()
         barrier()
         ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        ms /= args.e2e_steps
+        ms = max_over_ranks(ms, world, dev) / args.e2e_steps
         h2d = sum(t.numel() * 8 for t in (hB, hE, hO, hOm, hZ))
-        e2e = {"value": world * fl["F_min"] / (ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_build": ms, "steps": args.e2e_steps,
+        e2e = {"value": whole_job_value(fl["F_min"], world, ms), "unit": UNIT, "ms_per_build": ms, "steps": args.e2e_steps,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": hS.numel() * 8,
                "how": "qsgw_sigma_build_host from pinned host tensors; uploads overlap the kernels range by range"}
         assert torch.isfinite(hS).all()

@@ -244,11 +244,15 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
       double d[kTP / 16];
 #pragma unroll
       for (int j = 0; j < kTP / 16; ++j) d[j] = eps_p[j] - em;
+      // Omega_s of the next k-tile is fetched one k-tile ahead (a new 128-byte line per k-tile: an L2 round trip)
+      double om0n = __ldg(Omega + min(c2, s_c - 1)), om1n = __ldg(Omega + min(c2 + 1, s_c - 1));
 #pragma unroll 1
       for (int ks = 0; ks < KTS; ++ks, ++kt) {
         issue(kt + kAhead);
-        const int s = ks * kBK + c2;
-        const double om0 = __ldg(Omega + min(s, s_c - 1)), om1 = __ldg(Omega + min(s + 1, s_c - 1));
+        const double om0 = om0n, om1 = om1n;
+        const int sn = min(ks + 1, KTS - 1) * kBK + c2;
+        om0n = __ldg(Omega + min(sn, s_c - 1));
+        om1n = __ldg(Omega + min(sn + 1, s_c - 1));
         cp_async_wait<kAhead>();                  // this thread's copies of k-tile kt have landed
         double *rowA = smem + st * kSigmaStageDoubles + rA0 * kBK + csw;
         double2 cur[kTP / 16];
