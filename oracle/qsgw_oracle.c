@@ -33,6 +33,12 @@
  * power-of-two scaling, additivity over poles, eta->0 limit, null case, separable closed
  * form, permutation invariances, diagonal == G0W0 expression.
  *
+ * Next row, at the end of this file: qsgw_oracle_sigma_diag, the G0W0 diagonal Sigma_pp(omega) of
+ * Eq. (17) with m = n on a real frequency grid, complex.  Pins (tests/test_oracle_diag_pins.py): the
+ * same hand-solved two-state system on a grid in exact rationals (tests/golden/two_state_diag_grid.txt), literal
+ * Python-complex evaluation of Eq. (17) through the non-RI 4-index form, Re Sigma_pp(eps_p) == diagonal of the
+ * (separately pinned) qsGW matrix, exact power-of-two scaling, additivity over poles, sign of Im, eta -> 0 limit.
+ *
  * Floating point: products and the P-, ia- and m-sums are plain double; the running sum
  * over poles s of step 3 is kept in long double so that the oracle's own rounding is far
  * below the 1e-9 parity budget.
@@ -139,5 +145,54 @@ int qsgw_oracle_sigma(int N, int o, int naux, int64_t n_pole, const double *B, c
   }
   for (size_t k = 0; k < nS * nS; ++k) Sigma[k] = (double)acc[k];
   free(V); free(w); free(Dm); free(acc);
+  return 0;
+}
+
+/* ---- next row: G0W0 diagonal self-energy on a real frequency grid ------------------------
+ * "The conventional G0W0 method uses only diagonal elements (m = n) of Eq. (17)".  For the listed
+ * states p (states == NULL: all N) and the grid points omega[k], Eq. (17) with m = n = p, written out literally as a
+ * complex number (RI residues w of Eq. (18) as in steps 1-2 above):
+ *   Sigma_pp(omega) = sum_m sum_s w[s][p][m]^2 * ( occ[m] / (omega - eps[m] + Omega[s] - i eta)
+ *                                               + (1-occ[m]) / (omega - eps[m] - Omega[s] + i eta) )
+ * 1/(x - i eta) = (x + i eta)/(x^2+eta^2),  1/(x + i eta) = (x - i eta)/(x^2+eta^2).
+ * Re[r][k], Im[r][k] are n_states x n_omega, row-major.  Loop order: s outermost, w^s built, used, discarded; the
+ * pole sum is kept in long double.  Returns 0, or -1 on allocation failure / bad arguments. */
+int qsgw_oracle_sigma_diag(int N, int o, int naux, int64_t n_pole, const double *B, const double *eps,
+                           const double *occ, const double *Omega, const double *Z, int64_t ldz, double eta,
+                           int n_omega, const double *omega, int n_states, const int *states, double *Re, double *Im) {
+  if (N < 2 || o < 1 || o >= N || naux < 1 || n_pole < 1 || ldz < n_pole || !(eta > 0.0) || n_omega < 1) return -1;
+  if (!states) n_states = N;
+  if (n_states < 1) return -1;
+  const size_t nS = (size_t)n_states, nW = (size_t)n_omega;
+  double *V = (double *)malloc(sizeof(double) * (size_t)naux * (size_t)n_pole);
+  double *w = (double *)malloc(sizeof(double) * nS * N);
+  long double *accR = (long double *)malloc(sizeof(long double) * nS * nW);
+  long double *accI = (long double *)malloc(sizeof(long double) * nS * nW);
+  if (!V || !w || !accR || !accI) { free(V); free(w); free(accR); free(accI); return -1; }
+  for (size_t k = 0; k < nS * nW; ++k) accR[k] = accI[k] = 0.0L;
+
+  qsgw_oracle_pole_weights(N, o, naux, n_pole, B, Z, ldz, V, n_pole);            /* step 1 */
+
+  for (int64_t s = 0; s < n_pole; ++s) {
+    qsgw_oracle_residues(N, naux, B, V, n_pole, s, n_states, states, w);        /* step 2 */
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < n_states; ++r) {
+      for (int k = 0; k < n_omega; ++k) {
+        double tr = 0.0, ti = 0.0;
+        for (int m = 0; m < N; ++m) {
+          const double w2 = w[(size_t)r * N + m] * w[(size_t)r * N + m];
+          const double x1 = omega[k] - eps[m] + Omega[s];
+          const double x2 = omega[k] - eps[m] - Omega[s];
+          const double d1 = x1 * x1 + eta * eta, d2 = x2 * x2 + eta * eta;
+          tr += w2 * (occ[m] * (x1 / d1) + (1.0 - occ[m]) * (x2 / d2));
+          ti += w2 * (occ[m] * (eta / d1) - (1.0 - occ[m]) * (eta / d2));
+        }
+        accR[(size_t)r * nW + k] += (long double)tr;
+        accI[(size_t)r * nW + k] += (long double)ti;
+      }
+    }
+  }
+  for (size_t k = 0; k < nS * nW; ++k) { Re[k] = (double)accR[k]; Im[k] = (double)accI[k]; }
+  free(V); free(w); free(accR); free(accI);
   return 0;
 }

@@ -50,6 +50,9 @@ def _load():
         lib.qsgw_oracle_sigma.restype = ctypes.c_int
         lib.qsgw_oracle_sigma.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i64, dp, dp, dp, dp, dp, i64,
                                           ctypes.c_double, ctypes.c_int, ip, dp]
+        lib.qsgw_oracle_sigma_diag.restype = ctypes.c_int
+        lib.qsgw_oracle_sigma_diag.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i64, dp, dp, dp, dp, dp, i64,
+                                               ctypes.c_double, ctypes.c_int, dp, ctypes.c_int, ip, dp, dp]
         _lib = lib
     return _lib
 
@@ -129,3 +132,36 @@ def sigma(B, eps, occ, Omega, Z, eta: float, n_occ: int, states=None):
     if rc != 0:
         raise RuntimeError(f"qsgw_oracle_sigma failed with {rc}")
     return out
+
+
+def sigma_diag(B, eps, occ, Omega, Z, eta: float, n_occ: int, omega, states=None):
+    """G0W0 diagonal Sigma_pp(omega_k): Eq. (17) with m = n = p on a real frequency grid.
+
+    Returns (Re, Im), each [n_states, n_omega]; ``states`` (optional) lists the diagonal elements wanted.
+    """
+    B = _f64(B)
+    naux, N, N2 = B.shape
+    if N != N2:
+        raise ValueError("B must be [naux, N, N]")
+    eps = _f64(eps, (N,))
+    occ = _f64(occ, (N,))
+    Omega = _f64(Omega)
+    n_pole = Omega.shape[0]
+    Z = _f64(Z, (n_occ * (N - n_occ), n_pole))
+    omega = _f64(omega)
+    if omega.ndim != 1 or omega.shape[0] < 1:
+        raise ValueError("omega must be a non-empty 1-D grid")
+    if states is None:
+        n_states, sp, keep = N, None, None
+    else:
+        keep = np.ascontiguousarray(states, dtype=np.int32)
+        if keep.min() < 0 or keep.max() >= N:
+            raise ValueError("states out of range")
+        n_states, sp = len(keep), keep.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+    re = np.empty((n_states, omega.shape[0]))
+    im = np.empty((n_states, omega.shape[0]))
+    rc = _load().qsgw_oracle_sigma_diag(N, n_occ, naux, n_pole, _dp(B), _dp(eps), _dp(occ), _dp(Omega), _dp(Z),
+                                        n_pole, float(eta), omega.shape[0], _dp(omega), n_states, sp, _dp(re), _dp(im))
+    if rc != 0:
+        raise RuntimeError(f"qsgw_oracle_sigma_diag failed with {rc}")
+    return re, im
