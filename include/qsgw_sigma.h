@@ -59,6 +59,7 @@ typedef struct qsgw_sigma_stats {
   double ms_stage2;   int64_t launches_stage2;   /* w chunk = sqrt(2) B^T V           (DMMA GEMM)      */
   double ms_stage3;   int64_t launches_stage3;   /* T += (w.D) w^T                    (fused DMMA)     */
   double ms_epilogue; int64_t launches_epilogue; /* split-K reduce + symmetrise                         */
+  double ms_diag;     int64_t launches_diag;     /* G0W0 diagonal Sigma_pp(omega) kernel (qsgw_sigma_diag_build) */
   int64_t kernel_launches;                       /* CUDA kernels launched by the library (counted always) */
   int64_t builds;                                /* number of qsgw_sigma_finish calls                  */
   int64_t poles;                                 /* poles processed                                    */
@@ -120,6 +121,24 @@ int qsgw_sigma_finish(qsgw_sigma_plan *plan, double *Sigma);
 int qsgw_sigma_build_host(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ,
                           const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
                           double *Sigma);
+
+/*
+ * Next row of the scope table: the G0W0 diagonal self-energy on a real frequency grid,
+ *   Sigma_pp(omega_k) = sum_m sum_s w[s][p][m]^2 ( occ[m]     / (omega_k - eps[m] + Omega[s] - i eta)
+ *                                                + (1-occ[m]) / (omega_k - eps[m] - Omega[s] + i eta) ),
+ * i.e. Eq. (17) with m = n = p ("the conventional G0W0 method uses only diagonal elements"), for all
+ * n_mo states p and n_omega grid points.  Stages 1 and 2 (V and the s-blocked residues w) are those of qsgw_sigma_build;
+ * stage 3 is replaced by an FP64-ALU-bound reduction kernel.  Arguments as qsgw_sigma_build, plus
+ *   omega_grid device [n_omega]          real frequencies (Ha), n_omega >= 1
+ *   SigmaRe    device [n_mo][n_omega]    OVERWRITTEN with Re Sigma_pp(omega_k)
+ *   SigmaIm    device [n_mo][n_omega]    OVERWRITTEN with Im Sigma_pp(omega_k)
+ * Re Sigma_pp(eps[p]) equals the diagonal of the matrix qsgw_sigma_build returns (Eq. (19) with m = n).
+ * Asynchronous on the plan's stream.  INVALID_ARG as for qsgw_sigma_build, or if omega_grid / SigmaRe / SigmaIm is
+ * NULL or n_omega < 1, or if the chunk's Omega (s_block doubles) does not fit the kernel's shared memory (s_block > 24576).
+ */
+int qsgw_sigma_diag_build(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ,
+                          const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
+                          const double *omega_grid, int n_omega, double *SigmaRe, double *SigmaIm);
 
 /* Free the workspace and the plan.  Synchronises the plan's stream first.  NULL is accepted. */
 int qsgw_sigma_destroy(qsgw_sigma_plan *plan);

@@ -22,7 +22,7 @@ QSGW_SIGMA_ERR_CUDA = -3
 
 EXPORTS = (
     "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
-    "qsgw_sigma_build_host", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
+    "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
     "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_copy_workspace", "qsgw_sigma_version", "qsgw_sigma_fp64_probe",
 )
 
@@ -40,6 +40,7 @@ class qsgw_sigma_stats(ctypes.Structure):
         ("ms_stage2", ctypes.c_double), ("launches_stage2", ctypes.c_int64),
         ("ms_stage3", ctypes.c_double), ("launches_stage3", ctypes.c_int64),
         ("ms_epilogue", ctypes.c_double), ("launches_epilogue", ctypes.c_int64),
+        ("ms_diag", ctypes.c_double), ("launches_diag", ctypes.c_int64),
         ("kernel_launches", ctypes.c_int64), ("builds", ctypes.c_int64), ("poles", ctypes.c_int64),
     ]
 
@@ -72,6 +73,8 @@ def load_library() -> ctypes.CDLL:
         lib.qsgw_sigma_finish.argtypes = [vp, dp]
         lib.qsgw_sigma_build_host.restype = ci
         lib.qsgw_sigma_build_host.argtypes = [vp, dp, dp, dp, dp, dp, i64, i64, cd, dp]
+        lib.qsgw_sigma_diag_build.restype = ci
+        lib.qsgw_sigma_diag_build.argtypes = [vp, dp, dp, dp, dp, dp, i64, i64, cd, dp, ci, dp, dp]
         lib.qsgw_sigma_destroy.restype = ci
         lib.qsgw_sigma_destroy.argtypes = [vp]
         lib.qsgw_sigma_last_error.restype = ctypes.c_char_p
@@ -198,6 +201,25 @@ def qsgw_sigma_build_host(plan: Plan, B, eps, occ, Omega, Z, eta: float, Sigma: 
                                               _host(Sigma, "Sigma", (N, N)))
     _check(rc, plan.handle)
     return Sigma
+
+
+def qsgw_sigma_diag_build(plan: Plan, B, eps, occ, Omega, Z, eta: float, omega_grid, SigmaRe=None, SigmaIm=None):
+    """G0W0 diagonal Sigma_pp(omega_k) (Eq. (17) with m = n) for all states p; returns (Re, Im), each [n_mo, n_omega]."""
+    N = plan.n_mo
+    if not B.is_contiguous() or not eps.is_contiguous() or not occ.is_contiguous() or not omega_grid.is_contiguous():
+        raise ValueError("B, eps, occ, omega_grid must be contiguous")
+    n_omega = int(omega_grid.shape[0])
+    if SigmaRe is None:
+        SigmaRe = torch.empty((N, n_omega), dtype=torch.float64, device=B.device)
+    if SigmaIm is None:
+        SigmaIm = torch.empty((N, n_omega), dtype=torch.float64, device=B.device)
+    om, z, ldz, n_pole = _z_args(plan, Omega, Z, _dev)
+    rc = load_library().qsgw_sigma_diag_build(plan.handle, _dev(B, "B", (plan.n_aux, N, N)), _dev(eps, "eps", (N,)),
+                                              _dev(occ, "occ", (N,)), om, z, ldz, n_pole, float(eta),
+                                              _dev(omega_grid, "omega_grid", (n_omega,)), n_omega,
+                                              _dev(SigmaRe, "SigmaRe", (N, n_omega)), _dev(SigmaIm, "SigmaIm", (N, n_omega)))
+    _check(rc, plan.handle)
+    return SigmaRe, SigmaIm
 
 
 def _host_strided(t: torch.Tensor, name: str) -> int:

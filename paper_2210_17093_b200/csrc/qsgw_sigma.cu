@@ -24,7 +24,7 @@ namespace {
 
 thread_local std::string g_create_error;
 
-enum StageId { kPack = 0, kStage1, kStage2, kStage3, kEpilogue, kNumStages };
+enum StageId { kPack = 0, kStage1, kStage2, kStage3, kEpilogue, kDiag, kNumStages };
 
 struct EventPair {
   cudaEvent_t a, b;
@@ -63,8 +63,8 @@ struct qsgw_sigma_plan {
   bool profiling = false;
   std::vector<EventPair> pending[kNumStages];
   std::vector<EventPair> pool;
-  double ms[kNumStages] = {0, 0, 0, 0, 0};
-  int64_t launches[kNumStages] = {0, 0, 0, 0, 0};
+  double ms[kNumStages] = {0, 0, 0, 0, 0, 0};
+  int64_t launches[kNumStages] = {0, 0, 0, 0, 0, 0};
   int64_t builds = 0, poles = 0, kernel_launches = 0;
 
   std::string err;
@@ -184,7 +184,15 @@ int do_begin(qsgw_sigma_plan *p, const double *B, const double *eps, const doubl
   return QSGW_SIGMA_OK;
 }
 
-int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64_t ldz, int64_t n_pole) {
+struct DiagArgs {
+  const double *omega_grid;
+  int n_omega;
+  double *Re, *Im;
+};
+
+// diag == nullptr: stage 3 of the qsGW matrix; otherwise the G0W0 diagonal kernel takes its place
+int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64_t ldz, int64_t n_pole,
+                 const DiagArgs *diag = nullptr) {
   if (!p->begun) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles called before begin");
   if (!Omega || !Z) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles: Omega and Z must be non-NULL");
   if (n_pole < 1 || n_pole > p->n_pole_max)
@@ -218,7 +226,15 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
         int rc = launch_gemm<2>(p, p->Bp, p->ldp, p->V + c0, p->ldv, (int)p->n_pair, sc, p->n_aux, epi);
         if (rc) return rc;
       }
-      {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
+      if (diag) {  // G0W0 diagonal: Re/Im[p][k] += sum_m sum_{s in chunk} w^2 / (omega_k - eps_m +- Omega_s -+ i eta)
+        ScopedTimer t(p, kDiag);
+        const size_t smem = sizeof(double) * ((size_t)sc + (kDiagThreads / 32) * 2 * kDiagKW);
+        sigma_diag_kernel<<<dim3(p->n_mo, (diag->n_omega + kDiagKW - 1) / kDiagKW), kDiagThreads, smem, p->stream>>>(
+            p->W, p->ldw, p->eps, p->occ, Omega + v0 + c0, p->n_mo, sc, p->eta, diag->omega_grid, diag->n_omega,
+            diag->Re, diag->Im);
+        p->kernel_launches += 1;
+        QSGW_CUDA(p, cudaGetLastError());
+      } else {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
         ScopedTimer t(p, kStage3);
         sigma_accumulate_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
             p->W, p->ldw, p->eps, p->occ, Omega + v0 + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart);
@@ -378,6 +394,34 @@ int qsgw_sigma_build(qsgw_sigma_plan *p, const double *B, const double *eps, con
   return do_finish(p, Sigma);
 }
 
+int qsgw_sigma_diag_build(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ,
+                          const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
+                          const double *omega_grid, int n_omega, double *SigmaRe, double *SigmaIm) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  if (!Omega || !Z || !omega_grid || !SigmaRe || !SigmaIm) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: NULL argument");
+  if (n_pole < 1 || n_pole > p->n_pole_max) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: n_pole must be in [1, n_pole_max]");
+  if (ldz < n_pole) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: ldz < n_pole");
+  if (n_omega < 1) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: n_omega < 1");
+  const size_t smem_max = sizeof(double) * ((size_t)p->s_chunk + (kDiagThreads / 32) * 2 * kDiagKW);
+  if (smem_max > 200 * 1024) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: s_block too large for the diagonal kernel");
+  static bool configured = false;
+  if (!configured) {
+    QSGW_CUDA(p, cudaFuncSetAttribute(sigma_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    configured = true;
+  }
+  if ((rc = do_begin(p, B, eps, occ, eta))) return rc;
+  const size_t nbytes = sizeof(double) * (size_t)p->n_mo * n_omega;
+  QSGW_CUDA(p, cudaMemsetAsync(SigmaRe, 0, nbytes, p->stream));
+  QSGW_CUDA(p, cudaMemsetAsync(SigmaIm, 0, nbytes, p->stream));
+  DiagArgs diag{omega_grid, n_omega, SigmaRe, SigmaIm};
+  rc = do_add_poles(p, Omega, Z, ldz, n_pole, &diag);
+  p->begun = false;
+  if (rc) return rc;
+  p->builds += 1;
+  return QSGW_SIGMA_OK;
+}
+
 int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ,
                           const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
                           double *Sigma) {
@@ -486,6 +530,7 @@ int qsgw_sigma_get_stats(qsgw_sigma_plan *p, qsgw_sigma_stats *st, int reset) {
   st->ms_stage2 = p->ms[kStage2];     st->launches_stage2 = p->launches[kStage2];
   st->ms_stage3 = p->ms[kStage3];     st->launches_stage3 = p->launches[kStage3];
   st->ms_epilogue = p->ms[kEpilogue]; st->launches_epilogue = p->launches[kEpilogue];
+  st->ms_diag = p->ms[kDiag];         st->launches_diag = p->launches[kDiag];
   st->kernel_launches = p->kernel_launches;
   st->builds = p->builds;
   st->poles = p->poles;

@@ -376,4 +376,101 @@ __global__ void sigma_epilogue_kernel(const double *__restrict__ Tpart, int nspl
   }
 }
 
+// ---------------------------------------------------------------- next row: G0W0 diagonal on a frequency grid
+// Sigma_pp(omega_k) = sum_m sum_s w[s][p][m]^2 ( f_m / (omega_k - eps_m + Omega_s - i eta)
+//                                              + (1 - f_m) / (omega_k - eps_m - Omega_s + i eta) )
+// Eq. (17) with m = n = p, stages 1-2 unchanged.  No contraction is left: per (p, m, s, k) one
+// complex reciprocal, so the kernel is bound by the FP64 ALU rate (8 FP64-pipe instructions per evaluation:
+// x, y = x^2+eta^2, e, t, r (RCP64H seed + cubic correction as in stage 3), w^2 r, Re += (w^2 r) x, Im +-= w^2 r).
+// One CTA = one state p and kDiagKW grid points, all m and all s_c poles of the chunk; each element of w is loaded
+// once per CTA (coalesced along s) and used for kDiagKW evaluations.  The CTA owns its outputs and adds the chunk's
+// contribution to them with a plain read-modify-write: fixed order, reproducible, no atomics.
+constexpr int kDiagKW = 8;         // frequency points per thread
+constexpr int kDiagThreads = 128;
+
+__device__ __forceinline__ void diag_term(double x, double eta2, double w2, double wim, double &re, double &im) {
+  const double y = fma(x, x, eta2);
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
+  const double e = fma(-y, r, 1.0);
+  const double t = fma(e, e, e);
+  r = fma(r, t, r);                 // 1 / (x^2 + eta^2) to <= 1 ulp
+  re = fma(w2 * r, x, re);          // Re 1/(x -+ i eta) = x / (x^2 + eta^2)
+  im = fma(wim, r, im);             // Im 1/(x -+ i eta) = +-eta / (x^2 + eta^2); eta is applied once at the end
+}
+
+__global__ void __launch_bounds__(kDiagThreads)
+sigma_diag_kernel(const double *__restrict__ W, int64_t ldw, const double *__restrict__ eps,
+                  const double *__restrict__ occ, const double *__restrict__ Omega, int n_mo, int s_c, double eta,
+                  const double *__restrict__ omega_grid, int n_omega, double *__restrict__ Re, double *__restrict__ Im) {
+  extern __shared__ __align__(16) double smem[];     // [s_c] Omega of the chunk, then the cross-warp reduction scratch
+  double *om_s = smem;
+  double *red = smem + s_c;                          // [kDiagThreads / 32][2 * kDiagKW]
+  const int p = blockIdx.x, k0 = blockIdx.y * kDiagKW;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  for (int s = tid; s < s_c; s += kDiagThreads) om_s[s] = Omega[s];
+  double wk[kDiagKW], re[kDiagKW], im[kDiagKW];
+#pragma unroll
+  for (int k = 0; k < kDiagKW; ++k) {
+    wk[k] = __ldg(omega_grid + min(k0 + k, n_omega - 1));
+    re[k] = im[k] = 0.0;
+  }
+  __syncthreads();
+  const double eta2 = eta * eta;
+  for (int m = 0; m < n_mo; ++m) {
+    const double em = __ldg(eps + m), fo = __ldg(occ + m);
+    const long long fbits = __double_as_longlong(fo);
+    const int occ_class = (fbits == 0x3FF0000000000000LL) ? 1 : (((unsigned long long)fbits << 1) == 0ULL ? 0 : 2);
+    const double *row = W + ((int64_t)m * n_mo + p) * ldw;
+    if (occ_class != 2) {
+      const double sgn = occ_class == 1 ? 1.0 : -1.0;      // x = omega - eps_m + sgn Omega_s; Im carries the same sign
+      for (int s = tid; s < s_c; s += kDiagThreads) {
+        const double w = __ldg(row + s);
+        const double w2 = w * w, wim = sgn * w2;
+        const double b = fma(-sgn, om_s[s], em);           // eps_m - sgn Omega_s
+#pragma unroll
+        for (int k = 0; k < kDiagKW; ++k) diag_term(wk[k] - b, eta2, w2, wim, re[k], im[k]);
+      }
+    } else {
+      for (int s = tid; s < s_c; s += kDiagThreads) {
+        const double w = __ldg(row + s);
+        const double w2 = w * w;
+        const double b1 = em - om_s[s], b2 = em + om_s[s];
+#pragma unroll
+        for (int k = 0; k < kDiagKW; ++k) {
+          diag_term(wk[k] - b1, eta2, fo * w2, fo * w2, re[k], im[k]);
+          diag_term(wk[k] - b2, eta2, (1.0 - fo) * w2, -(1.0 - fo) * w2, re[k], im[k]);
+        }
+      }
+    }
+  }
+  // reduce over the CTA in a fixed order: butterfly inside each warp, then warps 0..3 in sequence
+#pragma unroll
+  for (int k = 0; k < kDiagKW; ++k) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      re[k] += __shfl_xor_sync(0xffffffffu, re[k], off);
+      im[k] += __shfl_xor_sync(0xffffffffu, im[k], off);
+    }
+  }
+  if (lane == 0) {
+#pragma unroll
+    for (int k = 0; k < kDiagKW; ++k) {
+      red[warp * 2 * kDiagKW + k] = re[k];
+      red[warp * 2 * kDiagKW + kDiagKW + k] = im[k];
+    }
+  }
+  __syncthreads();
+  if (tid < kDiagKW && k0 + tid < n_omega) {
+    double r = 0.0, i = 0.0;
+    for (int wv = 0; wv < kDiagThreads / 32; ++wv) {
+      r += red[wv * 2 * kDiagKW + tid];
+      i += red[wv * 2 * kDiagKW + kDiagKW + tid];
+    }
+    const int64_t o = (int64_t)p * n_omega + k0 + tid;
+    Re[o] += r;
+    Im[o] += eta * i;
+  }
+}
+
 }  // namespace qsgw
