@@ -346,6 +346,90 @@ def run_gpu(args):
     return 0
 
 
+def run_gpu_diag(args):
+    """--path diag: the next row of the scope table, measured to the same bar -- one step is one
+    qsgw_sigma_diag_build (pack, stage 1, stage 2 per s-block, the G0W0 diagonal kernel per s-block) for all N
+    states on an n_omega-point grid.  value = 1e9 complex Lehmann terms evaluated per second,
+    N^2 * n_s * n_omega / t; the kernel is bound by the FP64 ALU rate (8 FP64-pipe instructions per term)."""
+    import numpy as np
+    import torch
+    import qsgw_inputs as qi
+    import paper_2210_17093_b200 as pkg
+
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("--path diag is a single-GPU measurement")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    cfg = qi.CONFIGS[args.workload]
+    if cfg.name == "xl":
+        raise SystemExit("--path diag needs Z resident on the device: use tiny..large")
+    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+    pk, peak_src = _peaks()
+    lane_peak = nsm * FP64_FMA_PER_CLK_PER_SM * float(pk.get("sm_max_mhz", 1965.0)) * 1e6     # FP64 lane-instr / s
+    B = qi.make_B(cfg, dev)
+    eps, occ, Om = qi.make_eps(cfg).to(dev), qi.make_occ(cfg).to(dev), qi.make_omega(cfg).to(dev)
+    Z = qi.make_Z(cfg, device=dev)
+    lo, hi = float(eps.min()) - 1.0, float(eps.max()) + 1.0
+    grid = torch.linspace(lo, hi, args.n_omega, dtype=torch.float64, device=dev)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, cfg.s_block)
+    pkg.qsgw_sigma_set_profiling(plan, True)
+    Re = torch.empty((cfg.n_mo, args.n_omega), dtype=torch.float64, device=dev)
+    Im = torch.empty_like(Re)
+    for _ in range(args.warmup):
+        pkg.qsgw_sigma_diag_build(plan, B, eps, occ, Om, Z, cfg.eta, grid, Re, Im)
+    torch.cuda.synchronize()
+    pkg.qsgw_sigma_get_stats(plan, reset=True)
+    evs = []
+    with ClockSampler(0) as clocks:
+        torch.cuda.synchronize()
+        for _ in range(args.steps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); pkg.qsgw_sigma_diag_build(plan, B, eps, occ, Om, Z, cfg.eta, grid, Re, Im); e1.record()
+            evs.append((e0, e1))
+        torch.cuda.synchronize()
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    ms = sum(step_ms) / args.steps
+    stats = pkg.qsgw_sigma_get_stats(plan, reset=True)
+    assert torch.isfinite(Re).all() and torch.isfinite(Im).all()
+    terms = float(cfg.n_mo) ** 2 * cfg.n_pole * args.n_omega
+    nd = max(1, stats["launches_diag"])
+    d_ms = stats["ms_diag"] / nd
+    lane_instr = 8.0 * terms * args.steps / nd                      # FP64-pipe lane-instructions per diag launch
+    achieved = lane_instr / (d_ms * 1e-3)
+    out = {
+        "metric": "g0w0_diag_lehmann_terms_per_s", "value": terms / (ms * 1e-3) / 1e9, "unit": "Gterm/s", "n_gpus": 1,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "path": "diag (SURVEY.md 8(f).1, next row)",
+        "config": _config_dict(cfg, args, extra={"n_omega": args.n_omega, "grid": [lo, hi]}),
+        "stage_ms_per_build": {"pack": stats["ms_pack"] / args.steps, "stage1": stats["ms_stage1"] / args.steps,
+                               "stage2": stats["ms_stage2"] / args.steps, "diag": stats["ms_diag"] / args.steps},
+        "roofline": {"bound": "alu", "kernel": "sigma_diag_kernel", "achieved": achieved / 1e12, "peak": lane_peak / 1e12,
+                     "unit": "T FP64 lane-instr/s", "frac": achieved / lane_peak, "launches": stats["launches_diag"],
+                     "avg_launch_ms": d_ms, "traffic": None,
+                     "peak_source": f"{nsm} SMs x 64 FP64 lanes/clk x sm_max_mhz ({peak_src} MEASURED_PEAKS.json); a DFMA-only "
+                                    "loop reaches 80 % of it (profiles/r01_fp64_peaks.md); 8 FP64-pipe instructions per term"},
+        "gpu_launches": stats["kernel_launches"], "clocks": clocks.summary(),
+        "e2e": {"value": None, "unit": "Gterm/s", "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                "how": "no host-buffer entry point for this row yet"},
+    }
+    if not args.no_cpu_baseline:
+        import oracle
+        n_sample, states = max(4, min(cfg.n_pole, 64)), list(range(0, cfg.n_mo, max(1, cfg.n_mo // 16)))[:16]
+        t0 = time.perf_counter()
+        oracle.sigma_diag(B.cpu().numpy(), eps.cpu().numpy(), occ.cpu().numpy(), Om.cpu().numpy()[:n_sample],
+                          Z[:, :n_sample].cpu().numpy(), cfg.eta, cfg.n_occ, grid.cpu().numpy(), states=states)
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": len(states) * cfg.n_mo * n_sample * args.n_omega / dt / 1e9, "unit": "Gterm/s",
+                               "cores": oracle.num_threads(), "kind": "oracle",
+                               "sample": f"{len(states)} states x {n_sample} of {cfg.n_pole} poles x {args.n_omega} grid points "
+                                         f"of '{cfg.name}' ({dt:.1f} s, its steps 1-2 included)"}
+    print(json.dumps(out), flush=True)
+    pkg.qsgw_sigma_destroy(plan)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -359,11 +443,16 @@ def main():
     ap.add_argument("--e2e-warmup", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-poles", type=int, default=0, help="poles in the oracle's timed sample (0 = auto, ~20 s)")
+    ap.add_argument("--path", default="sigma", choices=["sigma", "diag"],
+                    help="sigma: the qsGW Sigma^c build (the bench contract); diag: the G0W0 diagonal on a frequency grid")
+    ap.add_argument("--n-omega", type=int, default=64, help="grid points of --path diag")
     args = ap.parse_args()
     if args.steps < 1 or args.warmup < 0:
         raise SystemExit("need --steps >= 1 and --warmup >= 0")
     if args.impl == "reference":
         return run_reference(args)
+    if args.path == "diag":
+        return run_gpu_diag(args)
     return run_gpu(args)
 
 
