@@ -165,3 +165,18 @@ def sigma_diag(B, eps, occ, Omega, Z, eta: float, n_occ: int, omega, states=None
     if rc != 0:
         raise RuntimeError(f"qsgw_oracle_sigma_diag failed with {rc}")
     return re, im
+
+
+def ao_to_mo(B_ao, C):
+    """RI AO->MO transformation of the three-index factors: the RI analogue of Eq. (16)
+    (RI remark PAPER.md:120), B^P_pq = sum_mu sum_nu C[mu][p] C[nu][q] B^P_mu,nu, i.e. for every
+    auxiliary function P the matrix identity B_mo[P] = C^T B_ao[P] C, written with numpy's FP64 matmul as the step.
+
+    B_ao [naux, nao, nao], C [nao, n_mo] (AO coefficients of the MOs, column p = orbital p) -> [naux, n_mo, n_mo].
+    Pinned in tests/test_oracle_aomo_pins.py against the literal 4-deep double sum on tiny inputs and invariants.
+    """
+    B_ao = _f64(B_ao)
+    C = _f64(C)
+    if B_ao.ndim != 3 or B_ao.shape[1] != B_ao.shape[2] or C.ndim != 2 or C.shape[0] != B_ao.shape[1]:
+        raise ValueError("need B_ao [naux, nao, nao] and C [nao, n_mo]")
+    return np.matmul(C.T[None, :, :], np.matmul(B_ao, C[None, :, :]))

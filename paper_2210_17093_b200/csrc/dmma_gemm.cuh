@@ -24,7 +24,6 @@ constexpr int kBM = 128;
 constexpr int kBN = 128;
 constexpr int kBK = 16;
 constexpr int kLdT = kBM + 4;   // k-major tile rows [k][128 + 4]: ld = 4 (mod 16) doubles -> LDS.64 fragments conflict-free
-constexpr int kLdK = kBK + 4;   // row-major tile rows [row][16 + 4]: same property for the [row][k] layout of stage 3
 constexpr int kGBK = 32;          // k depth of one ring stage of the stage-1/2 GEMM (two barrier round trips per 8 k4 steps cost ~2 %)
 constexpr int kGemmStages = 3;
 
@@ -40,10 +39,6 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)_
 
 __device__ __forceinline__ void cp_async_16(void *smem_dst, const void *gmem_src, int src_bytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(src_bytes)
-               : "memory");
-}
-__device__ __forceinline__ void cp_async_8(void *smem_dst, const void *gmem_src, int src_bytes) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(src_bytes)
                : "memory");
 }
 __device__ __forceinline__ void cp_async_16_s(uint32_t smem_dst, const void *gmem_src, int src_bytes) {
@@ -165,30 +160,6 @@ __device__ __forceinline__ void mma_ktile_kmajor_any(double (&acc)[8][4][2], con
     }
   } else {
     mma_ktile_kmajor<false>(acc, as, bs, fm);   // ragged in N too (last tile column of the last chunk): rare
-  }
-}
-
-// Same on row-major tiles As[row][kLdK], Bs[row][kLdK] (stage 3).
-template <bool FULL>
-__device__ __forceinline__ void mma_ktile_rowmajor(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
-  const double *ap = as + (8 * fm.wmi + fm.g) * kLdK + fm.t;
-  const double *bp = bs + (8 * fm.wni + fm.g) * kLdK + fm.t;
-#pragma unroll
-  for (int kk = 0; kk < kBK / 4; ++kk) {
-    double a[8], b[4];
-#pragma unroll
-    for (int i = 0; i < 8; ++i)
-      if (FULL || i < fm.mi_cnt) a[i] = ap[16 * i * kLdK + 4 * kk];
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-      if (FULL || j < fm.nj_cnt) b[j] = bp[32 * j * kLdK + 4 * kk];
-#pragma unroll
-    for (int i = 0; i < 8; ++i)
-      if (FULL || i < fm.mi_cnt) {
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-          if (FULL || j < fm.nj_cnt) dmma_m8n8k4(acc[i][j], a[i], b[j]);
-      }
   }
 }
 

@@ -1,0 +1,59 @@
+"""Pins of oracle.ao_to_mo (RI AO->MO transformation of B; RI analogue of Eq. (16))
+against things other than itself.  No CUDA path involved."""
+import numpy as np
+
+import oracle
+
+
+def _case(rng, naux, nao, n_mo, sym=True):
+    G = rng.normal(0, 1, (naux, nao, nao))
+    B = 0.5 * (G + G.transpose(0, 2, 1)) if sym else G
+    C = rng.normal(0, 1, (nao, n_mo))
+    return B, C
+
+
+def test_literal_double_sum_on_tiny_inputs():
+    """B^P_pq = sum_mu sum_nu C[mu][p] C[nu][q] B^P_mu,nu written as four nested Python loops; B NOT symmetric, nao != n_mo,
+    so a transposed operand or swapped index shows."""
+    rng = np.random.default_rng(1)
+    naux, nao, n_mo = 3, 5, 4
+    B, C = _case(rng, naux, nao, n_mo, sym=False)
+    want = np.zeros((naux, n_mo, n_mo))
+    for P in range(naux):
+        for p in range(n_mo):
+            for q in range(n_mo):
+                acc = 0.0
+                for mu in range(nao):
+                    for nu in range(nao):
+                        acc += C[mu, p] * C[nu, q] * B[P, mu, nu]
+                want[P, p, q] = acc
+    got = oracle.ao_to_mo(B, C)
+    assert got.shape == (naux, n_mo, n_mo)
+    assert np.max(np.abs(got - want)) <= 1e-13 * np.abs(want).max()
+
+
+def test_identity_permutation_and_selection():
+    rng = np.random.default_rng(2)
+    B, _ = _case(rng, 4, 6, 6)
+    assert np.array_equal(oracle.ao_to_mo(B, np.eye(6)), B)                      # C = 1
+    perm = rng.permutation(6)
+    Pm = np.eye(6)[:, perm]                                                     # orbital p = AO perm[p]
+    assert np.array_equal(oracle.ao_to_mo(B, Pm), B[:, perm][:, :, perm])
+    sel = np.eye(6)[:, [4, 1]]                                                  # two orbitals only: a 2 x 2 block
+    assert np.array_equal(oracle.ao_to_mo(B, sel), B[:, [4, 1]][:, :, [4, 1]])
+
+
+def test_composition_symmetry_linearity_and_trace():
+    rng = np.random.default_rng(3)
+    B, C1 = _case(rng, 3, 7, 7)
+    C2 = rng.normal(0, 1, (7, 5))
+    two_steps = oracle.ao_to_mo(oracle.ao_to_mo(B, C1), C2)
+    one_step = oracle.ao_to_mo(B, C1 @ C2)                                      # (C1 C2)^T B (C1 C2)
+    assert np.max(np.abs(two_steps - one_step)) <= 1e-12 * np.abs(one_step).max()
+    out = oracle.ao_to_mo(B, C1)
+    assert np.max(np.abs(out - out.transpose(0, 2, 1))) <= 1e-13 * np.abs(out).max()   # symmetric in, symmetric out
+    assert np.array_equal(oracle.ao_to_mo(2.0 * B, C1), 2.0 * out)              # linear in B (exact for a power of two)
+    assert np.array_equal(oracle.ao_to_mo(B, 2.0 * C1), 4.0 * out)              # quadratic in C
+    Q, _ = np.linalg.qr(rng.normal(0, 1, (7, 7)))                               # orthogonal C preserves the trace
+    tr = np.trace(oracle.ao_to_mo(B, Q), axis1=1, axis2=2)
+    assert np.max(np.abs(tr - np.trace(B, axis1=1, axis2=2))) <= 1e-12 * np.abs(B).max() * 7
