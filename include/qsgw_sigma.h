@@ -140,6 +140,24 @@ int qsgw_sigma_diag_build(qsgw_sigma_plan *plan, const double *B, const double *
                           const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
                           const double *omega_grid, int n_omega, double *SigmaRe, double *SigmaIm);
 
+/*
+ * Row 8(f).2 of the scope table: the RI AO->MO transformation that produces the B argument of the calls above, once per
+ * qsGW iteration (the RI analogue of Eq. (16); RI remark PAPER.md:120):
+ *   B_mo[P][p][q] = sum_mu sum_nu C[mu][p] * C[nu][q] * B_ao[P][mu][nu]        (B_mo[P] = C^T B_ao[P] C)
+ * as two batched FP64 tensor-core GEMMs over the n_aux auxiliary functions (half transform into `work`, then the second
+ * index).  No plan is needed.
+ *   B_ao  device [n_aux][n_ao][n_ao]   three-index RI factors in the AO basis (need not be symmetric)
+ *   C     device [n_ao][n_mo]          AO coefficients of the MOs, column p = orbital p
+ *   work  device, qsgw_ri_ao_to_mo_work_doubles(n_aux, n_ao, n_mo) doubles, 16-byte aligned; caller-owned scratch
+ *   B_mo  device [n_aux][n_mo][n_mo]   OVERWRITTEN
+ *   cuda_stream  a cudaStream_t or NULL; the call is asynchronous on it
+ * Errors: INVALID_ARG for NULL pointers, sizes < 1 or a misaligned work buffer; CUDA if no sm_100 device or a launch fails
+ * (message: qsgw_sigma_last_error(NULL)).
+ */
+int qsgw_ri_ao_to_mo(const double *B_ao, const double *C, int n_aux, int n_ao, int n_mo, double *work, double *B_mo,
+                     void *cuda_stream);
+size_t qsgw_ri_ao_to_mo_work_doubles(int n_aux, int n_ao, int n_mo);
+
 /* Free the workspace and the plan.  Synchronises the plan's stream first.  NULL is accepted. */
 int qsgw_sigma_destroy(qsgw_sigma_plan *plan);
 

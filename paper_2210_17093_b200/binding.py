@@ -22,7 +22,7 @@ QSGW_SIGMA_ERR_CUDA = -3
 
 EXPORTS = (
     "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
-    "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
+    "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_ri_ao_to_mo", "qsgw_ri_ao_to_mo_work_doubles", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
     "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_copy_workspace", "qsgw_sigma_version", "qsgw_sigma_fp64_probe",
 )
 
@@ -75,6 +75,10 @@ def load_library() -> ctypes.CDLL:
         lib.qsgw_sigma_build_host.argtypes = [vp, dp, dp, dp, dp, dp, i64, i64, cd, dp]
         lib.qsgw_sigma_diag_build.restype = ci
         lib.qsgw_sigma_diag_build.argtypes = [vp, dp, dp, dp, dp, dp, i64, i64, cd, dp, ci, dp, dp]
+        lib.qsgw_ri_ao_to_mo.restype = ci
+        lib.qsgw_ri_ao_to_mo.argtypes = [dp, dp, ci, ci, ci, dp, dp, vp]
+        lib.qsgw_ri_ao_to_mo_work_doubles.restype = ctypes.c_size_t
+        lib.qsgw_ri_ao_to_mo_work_doubles.argtypes = [ci, ci, ci]
         lib.qsgw_sigma_destroy.restype = ci
         lib.qsgw_sigma_destroy.argtypes = [vp]
         lib.qsgw_sigma_last_error.restype = ctypes.c_char_p
@@ -220,6 +224,33 @@ def qsgw_sigma_diag_build(plan: Plan, B, eps, occ, Omega, Z, eta: float, omega_g
                                               _dev(SigmaRe, "SigmaRe", (N, n_omega)), _dev(SigmaIm, "SigmaIm", (N, n_omega)))
     _check(rc, plan.handle)
     return SigmaRe, SigmaIm
+
+
+def qsgw_ri_ao_to_mo_work_doubles(n_aux: int, n_ao: int, n_mo: int) -> int:
+    return int(load_library().qsgw_ri_ao_to_mo_work_doubles(int(n_aux), int(n_ao), int(n_mo)))
+
+
+def qsgw_ri_ao_to_mo(B_ao: torch.Tensor, C: torch.Tensor, B_mo: Optional[torch.Tensor] = None,
+                     work: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """B_mo[P] = C^T B_ao[P] C for every auxiliary function P (RI AO->MO transformation); asynchronous on the stream."""
+    if B_ao.dim() != 3 or B_ao.shape[1] != B_ao.shape[2] or C.dim() != 2 or C.shape[0] != B_ao.shape[1]:
+        raise ValueError("need B_ao [n_aux, n_ao, n_ao] and C [n_ao, n_mo]")
+    if not B_ao.is_contiguous() or not C.is_contiguous():
+        raise ValueError("B_ao and C must be contiguous")
+    n_aux, n_ao, n_mo = int(B_ao.shape[0]), int(B_ao.shape[1]), int(C.shape[1])
+    if B_mo is None:
+        B_mo = torch.empty((n_aux, n_mo, n_mo), dtype=torch.float64, device=B_ao.device)
+    need = qsgw_ri_ao_to_mo_work_doubles(n_aux, n_ao, n_mo)
+    if work is None:
+        work = torch.empty(need, dtype=torch.float64, device=B_ao.device)
+    if work.numel() < need or not work.is_contiguous():
+        raise ValueError(f"work needs {need} contiguous doubles")
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    rc = load_library().qsgw_ri_ao_to_mo(_dev(B_ao, "B_ao"), _dev(C, "C"), n_aux, n_ao, n_mo, _dev(work, "work"),
+                                         _dev(B_mo, "B_mo", (n_aux, n_mo, n_mo)), ctypes.c_void_p(stream.cuda_stream))
+    _check(rc, None)
+    return B_mo
 
 
 def _host_strided(t: torch.Tensor, name: str) -> int:

@@ -201,16 +201,19 @@ __device__ __forceinline__ void load_tile_kmajor(double *dst, const double *src,
 }
 
 // ---------------------------------------------------------------- epilogues
-// C[row][col] = alpha * acc   (stage 1: V)
+// C[row][col] = alpha * acc   (stage 1: V, alpha = 1; AO->MO half transforms); batch b writes at C + b * strideC.
 struct EpiStore {
   double *C;
   int64_t ldc;
   double alpha;
+  int64_t strideC;   // doubles between the outputs of consecutive batches (0 when there is one batch)
+  int vec;           // 1: C 16-byte aligned, ldc and strideC even -> double2 stores
   using RowCtx = int;
+  __device__ __forceinline__ EpiStore for_batch(int b) const { return EpiStore{C + (int64_t)b * strideC, ldc, alpha, 0, vec}; }
   __device__ __forceinline__ RowCtx row_ctx(int) const { return 0; }
   __device__ __forceinline__ void operator()(RowCtx, int row, int col, double v0, double v1, int ncols) const {
     double *dst = C + (int64_t)row * ldc + col;
-    if (col + 1 < ncols && ((ldc & 1) == 0)) {
+    if (vec && col + 1 < ncols) {
       *reinterpret_cast<double2 *>(dst) = make_double2(alpha * v0, alpha * v1);
     } else {
       dst[0] = alpha * v0;
@@ -228,6 +231,7 @@ struct EpiPairScatter {
   int n_mo;
   double alpha;
   using RowCtx = int2;
+  __device__ __forceinline__ EpiPairScatter for_batch(int) const { return *this; }
   __device__ __forceinline__ RowCtx row_ctx(int row) const { return __ldg(pairs + row); }
   __device__ __forceinline__ void operator()(RowCtx pm, int, int col, double v0, double v1, int ncols) const {
     double *d0 = W + ((int64_t)pm.y * n_mo + pm.x) * ldw + col;
@@ -247,13 +251,14 @@ struct EpiPairScatter {
 constexpr size_t kGemmSmemBytes = (size_t)kGemmStages * 2 * kGBK * kLdT * sizeof(double) + 2 * kGemmStages * sizeof(uint64_t);
 
 // C(M x N) = epilogue( sum_k A[k][m] * B[k][n] ),  A stored [K][lda] (m contiguous), B stored [K][ldb] (n contiguous).
-// A must be 16-byte aligned with even lda (library workspace); B may be arbitrary when VECB == 1.
+// VECA / VECB = 2 need the operand 16-byte aligned with even leading dimension (and even batch stride); 1 takes anything.
+// nbatch independent problems of the same shape (operands strideA / strideB doubles apart, 0 = shared) share one launch.
 // ntm * ntn tiles of 128 x 128 dealt round-robin to the grid; m_fastest picks which tile index varies fastest (the
 // dimension with fewer tiles, so that concurrently running CTAs share operand panels in L2).
-template <int VECB, class Epi>
+template <int VECA, int VECB, class Epi>
 __global__ void __launch_bounds__(kThreads, 1)
-gemm_tn_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__restrict__ Bm, int64_t ldb, int M, int N,
-                    int K, int ntm, int ntn, int m_fastest, Epi epi) {
+gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__restrict__ B0, int64_t ldb, int M, int N,
+                    int K, int ntm, int ntn, int m_fastest, int nbatch, int64_t strideA, int64_t strideB, Epi epi0) {
   extern __shared__ __align__(16) double smem[];
   double *As = smem;
   double *Bs = smem + kGemmStages * kGBK * kLdT;
@@ -261,7 +266,8 @@ gemm_tn_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__r
   uint64_t *empty = full + kGemmStages;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int KT = (K + kGBK - 1) / kGBK;
-  const int ntiles = ntm * ntn;
+  const int tiles_per_batch = ntm * ntn;
+  const int ntiles = tiles_per_batch * nbatch;
 
   if (tid == 0) {
     for (int s = 0; s < kGemmStages; ++s) {
@@ -282,14 +288,16 @@ gemm_tn_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__r
     int st = 0;
     uint32_t ph = 1;   // a fresh barrier passes a wait on parity 1: the first pass over the ring does not block
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      const int batch = tile / tiles_per_batch, t = tile - batch * tiles_per_batch;
       int tm, tn;
-      if (m_fastest) { tn = tile / ntm; tm = tile - tn * ntm; }
-      else { tm = tile / ntn; tn = tile - tm * ntn; }
+      if (m_fastest) { tn = t / ntm; tm = t - tn * ntm; }
+      else { tm = t / ntn; tn = t - tm * ntn; }
       const int m0 = tm * kBM, n0 = tn * kBN;
+      const double *A = A0 + batch * strideA, *Bm = B0 + batch * strideB;
       for (int kt = 0; kt < KT; ++kt) {
         mbar_wait(empty + st, ph);
         const int k0 = kt * kGBK;
-        load_tile_kmajor<2>(As + st * kGBK * kLdT, A + (int64_t)k0 * lda + m0, lda, K - k0, M - m0, A, pt);
+        load_tile_kmajor<VECA>(As + st * kGBK * kLdT, A + (int64_t)k0 * lda + m0, lda, K - k0, M - m0, A, pt);
         load_tile_kmajor<VECB>(Bs + st * kGBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, K - k0, N - n0, Bm, pt);
         cp_async_mbar_arrive_noinc(full + st);
         if (++st == kGemmStages) { st = 0; ph ^= 1; }
@@ -302,10 +310,12 @@ gemm_tn_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__r
     int st = 0;
     uint32_t ph = 0;
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      const int batch = tile / tiles_per_batch, t = tile - batch * tiles_per_batch;
       int tm, tn;
-      if (m_fastest) { tn = tile / ntm; tm = tile - tn * ntm; }
-      else { tm = tile / ntn; tn = tile - tm * ntn; }
+      if (m_fastest) { tn = t / ntm; tm = t - tn * ntm; }
+      else { tm = t / ntn; tn = t - tm * ntn; }
       const int m0 = tm * kBM, n0 = tn * kBN;
+      const Epi epi = epi0.for_batch(batch);
       const FragMap fm(warp, lane, M - m0, N - n0);
       const bool full_tile = fm.mi_cnt == 8 && fm.nj_cnt == 4;
       // per-row epilogue context (stage 2: the (p, m) pair of the row), fetched now so its latency hides behind the k loop

@@ -138,23 +138,31 @@ void drain_events(qsgw_sigma_plan *p) {
   }
 }
 
-template <int VECB, class Epi>
-int launch_gemm(qsgw_sigma_plan *p, const double *A, int64_t lda, const double *Bm, int64_t ldb, int M, int N, int K,
-                const Epi &epi) {
+template <int VECA, int VECB, class Epi>
+int launch_gemm_on(qsgw_sigma_plan *p, cudaStream_t stream, int num_sms, const double *A, int64_t lda, const double *Bm,
+                   int64_t ldb, int M, int N, int K, const Epi &epi, int nbatch, int64_t strideA, int64_t strideB) {
   static bool configured = false;
-  auto kern = gemm_tn_dmma_kernel<VECB, Epi>;
+  auto kern = gemm_tn_dmma_kernel<VECA, VECB, Epi>;
   if (!configured) {
     QSGW_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGemmSmemBytes));
     configured = true;
   }
   const int ntm = (M + kBM - 1) / kBM, ntn = (N + kBN - 1) / kBN;
-  if ((int64_t)ntm * ntn > INT32_MAX) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "GEMM grid too large");
-  // the dimension with fewer tiles varies fastest: the CTAs of one wave then share its few operand panels in L2
-  // persistent: one CTA per SM walks the tiles round-robin
-  kern<<<std::min(ntm * ntn, p->num_sms), kThreads, kGemmSmemBytes, p->stream>>>(A, lda, Bm, ldb, M, N, K, ntm, ntn, ntm <= ntn ? 1 : 0, epi);
-  p->kernel_launches += 1;
+  if ((int64_t)ntm * ntn * nbatch > INT32_MAX) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "GEMM grid too large");
+  // persistent: one CTA per SM walks the tiles round-robin; the dimension with fewer tiles varies fastest, so that the
+  // CTAs running at the same time share its few operand panels in L2
+  kern<<<std::min(ntm * ntn * nbatch, num_sms), kThreads, kGemmSmemBytes, stream>>>(
+      A, lda, Bm, ldb, M, N, K, ntm, ntn, ntm <= ntn ? 1 : 0, nbatch, strideA, strideB, epi);
   QSGW_CUDA(p, cudaGetLastError());
   return QSGW_SIGMA_OK;
+}
+
+template <int VECB, class Epi>
+int launch_gemm(qsgw_sigma_plan *p, const double *A, int64_t lda, const double *Bm, int64_t ldb, int M, int N, int K,
+                const Epi &epi) {
+  int rc = launch_gemm_on<2, VECB>(p, p->stream, p->num_sms, A, lda, Bm, ldb, M, N, K, epi, 1, 0, 0);
+  if (rc == QSGW_SIGMA_OK) p->kernel_launches += 1;
+  return rc;
 }
 
 inline bool aligned16(const void *ptr, int64_t ld) { return (reinterpret_cast<uintptr_t>(ptr) & 15) == 0 && (ld & 1) == 0; }
@@ -211,7 +219,7 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
     {  // stage 1 for all poles of this range at once (enough tiles to fill the SMs evenly):
        // V[P][s] = sum_ia BovT[ia][P] * Z[ia][v0+s]
       ScopedTimer t(p, kStage1);
-      EpiStore epi{p->V, p->ldv, 1.0};
+      EpiStore epi{p->V, p->ldv, 1.0, 0, 1};   // V: library workspace, 16-byte aligned, even ldv
       const double *Zc = Z + v0;
       int rc = aligned16(Zc, ldz)
                    ? launch_gemm<2>(p, p->BovT, p->ld_aux, Zc, ldz, p->n_aux, (int)nv, (int)p->n_ov, epi)
@@ -465,6 +473,49 @@ int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps
   if ((rc = do_finish(p, p->hSigma))) return rc;
   QSGW_CUDA(p, cudaMemcpyAsync(Sigma, p->hSigma, sizeof(double) * nn, cudaMemcpyDeviceToHost, p->stream));
   QSGW_CUDA(p, cudaStreamSynchronize(p->stream));
+  return QSGW_SIGMA_OK;
+}
+
+size_t qsgw_ri_ao_to_mo_work_doubles(int n_aux, int n_ao, int n_mo) {
+  if (n_aux < 1 || n_ao < 1 || n_mo < 1) return 0;
+  return (size_t)n_aux * (size_t)n_ao * (size_t)round_up(n_mo, 2);
+}
+
+int qsgw_ri_ao_to_mo(const double *B_ao, const double *C, int n_aux, int n_ao, int n_mo, double *work, double *B_mo,
+                     void *cuda_stream) {
+  if (!B_ao || !C || !work || !B_mo) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "ao_to_mo: NULL argument");
+  if (n_aux < 1 || n_ao < 1 || n_mo < 1) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "ao_to_mo: sizes must be >= 1");
+  if (reinterpret_cast<uintptr_t>(work) & 15) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "ao_to_mo: work must be 16-byte aligned");
+  int dev = 0, sms = 0, major = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, QSGW_SIGMA_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
+  }
+  if (major != 10) return fail(nullptr, QSGW_SIGMA_ERR_CUDA, "this library is built for sm_100a (B200) only");
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const int64_t ldt = round_up(n_mo, 2);
+  const int64_t sB = (int64_t)n_ao * n_ao, sT = (int64_t)n_ao * ldt, sO = (int64_t)n_mo * n_mo;
+  const bool vC = aligned16(C, n_mo);
+  // step 1 (second index): work[P][nu][p] = sum_mu B_ao[P][mu][nu] * C[mu][p]     A = B_ao[P] (k = mu, m = nu), B = C
+  {
+    EpiStore epi{work, ldt, 1.0, sT, 1};
+    const bool vA = aligned16(B_ao, n_ao) && (sB & 1) == 0;
+    int rc = vA ? (vC ? launch_gemm_on<2, 2>(nullptr, stream, sms, B_ao, n_ao, C, n_mo, n_ao, n_mo, n_ao, epi, n_aux, sB, 0)
+                      : launch_gemm_on<2, 1>(nullptr, stream, sms, B_ao, n_ao, C, n_mo, n_ao, n_mo, n_ao, epi, n_aux, sB, 0))
+                : (vC ? launch_gemm_on<1, 2>(nullptr, stream, sms, B_ao, n_ao, C, n_mo, n_ao, n_mo, n_ao, epi, n_aux, sB, 0)
+                      : launch_gemm_on<1, 1>(nullptr, stream, sms, B_ao, n_ao, C, n_mo, n_ao, n_mo, n_ao, epi, n_aux, sB, 0));
+    if (rc) return rc;
+  }
+  // step 2 (first index): B_mo[P][p][q] = sum_nu work[P][nu][p] * C[nu][q]        A = work[P] (k = nu, m = p), B = C
+  {
+    EpiStore epi{B_mo, n_mo, 1.0, sO, (aligned16(B_mo, n_mo) && (sO & 1) == 0) ? 1 : 0};
+    int rc = vC ? launch_gemm_on<2, 2>(nullptr, stream, sms, work, ldt, C, n_mo, n_mo, n_mo, n_ao, epi, n_aux, sT, 0)
+                : launch_gemm_on<2, 1>(nullptr, stream, sms, work, ldt, C, n_mo, n_mo, n_mo, n_ao, epi, n_aux, sT, 0);
+    if (rc) return rc;
+  }
   return QSGW_SIGMA_OK;
 }
 
