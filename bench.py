@@ -430,6 +430,64 @@ def run_gpu_diag(args):
     return 0
 
 
+def run_gpu_aomo(args):
+    """--path aomo: row 8(f).2, B_mo[P] = C^T B_ao[P] C for all naux auxiliary functions of the workload
+    (two batched DMMA GEMMs, 4 N^3 naux flops); value in FP64 TFLOP/s against the same tensor roofline."""
+    import torch
+    import qsgw_inputs as qi
+    import paper_2210_17093_b200 as pkg
+
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("--path aomo is a single-GPU measurement")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    cfg = qi.CONFIGS[args.workload]
+    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak, peak_src, _ = fp64_peak_tflops(nsm)
+    B_ao = qi.make_B(cfg, dev)                                   # the config's B stands in for the AO-basis factors
+    g = torch.Generator(device=dev); g.manual_seed(cfg.seed)
+    C, _ = torch.linalg.qr(torch.randn((cfg.n_mo, cfg.n_mo), generator=g, dtype=torch.float64, device=dev))
+    C = C.contiguous()
+    work = torch.empty(pkg.qsgw_ri_ao_to_mo_work_doubles(cfg.n_aux, cfg.n_mo, cfg.n_mo), dtype=torch.float64, device=dev)
+    B_mo = torch.empty_like(B_ao)
+    for _ in range(args.warmup):
+        pkg.qsgw_ri_ao_to_mo(B_ao, C, B_mo, work)
+    torch.cuda.synchronize()
+    evs = []
+    with ClockSampler(0) as clocks:
+        for _ in range(args.steps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); pkg.qsgw_ri_ao_to_mo(B_ao, C, B_mo, work); e1.record()
+            evs.append((e0, e1))
+        torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps
+    flops = 4.0 * float(cfg.n_mo) ** 3 * cfg.n_aux
+    val = flops / (ms * 1e-3) / 1e12
+    assert torch.isfinite(B_mo).all()
+    out = {"metric": "ri_ao_to_mo_fp64_tflops", "value": val, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic", "path": "aomo (SURVEY.md 8(f).2, next row)",
+           "config": _config_dict(cfg, args, extra={"n_ao": cfg.n_mo, "flops": flops}),
+           "roofline": {"bound": "tensor", "kernel": "gemm_tn_dmma_kernel<*,*,EpiStore> (two batched launches)",
+                        "achieved": val, "peak": peak, "unit": UNIT, "frac": val / peak, "launches": 2 * args.steps,
+                        "avg_launch_ms": ms / 2, "traffic": None, "peak_source": f"FP64 pipe rate at max SM clock ({peak_src})"},
+           "gpu_launches": 2 * args.steps, "clocks": clocks.summary(),
+           "e2e": {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                   "how": "B stays on the device between the transform and the Sigma build"}}
+    if not args.no_cpu_baseline:
+        import oracle
+        n_s = min(cfg.n_aux, 64)
+        t0 = time.perf_counter()
+        oracle.ao_to_mo(B_ao[:n_s].cpu().numpy(), C.cpu().numpy())
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": 4.0 * float(cfg.n_mo) ** 3 * n_s / dt / 1e12, "unit": UNIT, "cores": os.cpu_count(),
+                               "kind": "oracle", "sample": f"{n_s} of {cfg.n_aux} auxiliary functions of '{cfg.name}' ({dt:.2f} s; numpy matmul)"}
+    print(json.dumps(out), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -443,7 +501,7 @@ def main():
     ap.add_argument("--e2e-warmup", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-poles", type=int, default=0, help="poles in the oracle's timed sample (0 = auto, ~20 s)")
-    ap.add_argument("--path", default="sigma", choices=["sigma", "diag"],
+    ap.add_argument("--path", default="sigma", choices=["sigma", "diag", "aomo"],
                     help="sigma: the qsGW Sigma^c build (the bench contract); diag: the G0W0 diagonal on a frequency grid")
     ap.add_argument("--n-omega", type=int, default=64, help="grid points of --path diag")
     args = ap.parse_args()
@@ -453,6 +511,8 @@ def main():
         return run_reference(args)
     if args.path == "diag":
         return run_gpu_diag(args)
+    if args.path == "aomo":
+        return run_gpu_aomo(args)
     return run_gpu(args)
 
 

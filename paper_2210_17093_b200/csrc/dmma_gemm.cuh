@@ -99,67 +99,49 @@ struct FragMap {
   __device__ __forceinline__ int out_col(int j) const { return 32 * j + 8 * wni + 2 * t; }  // first of this lane's 2 accumulator columns
 };
 
-// One k-tile (kGBK deep) of DMMA work on k-major tiles As[k][kLdT], Bs[k][kLdT].
-template <bool FULL>
-__device__ __forceinline__ void mma_ktile_kmajor(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
+// The first MI x NJ fragments of the warp, MI and NJ compile-time constants -- a predicated-off DMMA still costs its pipe
+// time, so the fragments a warp does not own in a ragged tile must be branched around, not predicated.
+template <int MI, int NJ>
+__device__ __forceinline__ void mma_ktile_kmajor_frag(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
   const double *ap = as + 8 * fm.wmi + fm.g + fm.t * kLdT;
   const double *bp = bs + 8 * fm.wni + fm.g + fm.t * kLdT;
 #pragma unroll
   for (int kk = 0; kk < kGBK / 4; ++kk) {
-    double a[8], b[4];
-#pragma unroll
-    for (int i = 0; i < 8; ++i)
-      if (FULL || i < fm.mi_cnt) a[i] = ap[kk * 4 * kLdT + 16 * i];
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-      if (FULL || j < fm.nj_cnt) b[j] = bp[kk * 4 * kLdT + 32 * j];
-#pragma unroll
-    for (int i = 0; i < 8; ++i)
-      if (FULL || i < fm.mi_cnt) {
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-          if (FULL || j < fm.nj_cnt) dmma_m8n8k4(acc[i][j], a[i], b[j]);
-      }
-  }
-}
-
-// Ragged in M only (the last row of tiles of stage 1 / stage 2): the first MI row fragments, all 4 column fragments,
-// with MI a compile-time constant -- a predicated-off DMMA still costs its pipe time, so the fragments a warp does not
-// own must be branched around, not predicated.
-template <int MI>
-__device__ __forceinline__ void mma_ktile_kmajor_rows(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
-  const double *ap = as + 8 * fm.wmi + fm.g + fm.t * kLdT;
-  const double *bp = bs + 8 * fm.wni + fm.g + fm.t * kLdT;
-#pragma unroll
-  for (int kk = 0; kk < kGBK / 4; ++kk) {
-    double a[MI], b[4];
+    double a[MI], b[NJ];
 #pragma unroll
     for (int i = 0; i < MI; ++i) a[i] = ap[kk * 4 * kLdT + 16 * i];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) b[j] = bp[kk * 4 * kLdT + 32 * j];
+    for (int j = 0; j < NJ; ++j) b[j] = bp[kk * 4 * kLdT + 32 * j];
 #pragma unroll
     for (int i = 0; i < MI; ++i)
 #pragma unroll
-      for (int j = 0; j < 4; ++j) dmma_m8n8k4(acc[i][j], a[i], b[j]);
+      for (int j = 0; j < NJ; ++j) dmma_m8n8k4(acc[i][j], a[i], b[j]);
   }
 }
 
-// Dispatch of one k-tile on the (warp-uniform) fragment counts of the tile.
+template <int NJ>
+__device__ __forceinline__ void mma_ktile_kmajor_mi(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
+  switch (fm.mi_cnt) {
+    case 8: mma_ktile_kmajor_frag<8, NJ>(acc, as, bs, fm); break;
+    case 7: mma_ktile_kmajor_frag<7, NJ>(acc, as, bs, fm); break;
+    case 6: mma_ktile_kmajor_frag<6, NJ>(acc, as, bs, fm); break;
+    case 5: mma_ktile_kmajor_frag<5, NJ>(acc, as, bs, fm); break;
+    case 4: mma_ktile_kmajor_frag<4, NJ>(acc, as, bs, fm); break;
+    case 3: mma_ktile_kmajor_frag<3, NJ>(acc, as, bs, fm); break;
+    case 2: mma_ktile_kmajor_frag<2, NJ>(acc, as, bs, fm); break;
+    case 1: mma_ktile_kmajor_frag<1, NJ>(acc, as, bs, fm); break;
+    default: break;
+  }
+}
+
+// Dispatch of one k-tile on the (warp-uniform) fragment counts of a ragged tile.
 __device__ __forceinline__ void mma_ktile_kmajor_any(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
-  if (fm.nj_cnt == 4) {
-    switch (fm.mi_cnt) {
-      case 8: mma_ktile_kmajor_rows<8>(acc, as, bs, fm); break;
-      case 7: mma_ktile_kmajor_rows<7>(acc, as, bs, fm); break;
-      case 6: mma_ktile_kmajor_rows<6>(acc, as, bs, fm); break;
-      case 5: mma_ktile_kmajor_rows<5>(acc, as, bs, fm); break;
-      case 4: mma_ktile_kmajor_rows<4>(acc, as, bs, fm); break;
-      case 3: mma_ktile_kmajor_rows<3>(acc, as, bs, fm); break;
-      case 2: mma_ktile_kmajor_rows<2>(acc, as, bs, fm); break;
-      case 1: mma_ktile_kmajor_rows<1>(acc, as, bs, fm); break;
-      default: break;
-    }
-  } else {
-    mma_ktile_kmajor<false>(acc, as, bs, fm);   // ragged in N too (last tile column of the last chunk): rare
+  switch (fm.nj_cnt) {
+    case 4: mma_ktile_kmajor_mi<4>(acc, as, bs, fm); break;
+    case 3: mma_ktile_kmajor_mi<3>(acc, as, bs, fm); break;
+    case 2: mma_ktile_kmajor_mi<2>(acc, as, bs, fm); break;
+    case 1: mma_ktile_kmajor_mi<1>(acc, as, bs, fm); break;
+    default: break;
   }
 }
 
@@ -330,7 +312,7 @@ gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__
 #pragma unroll 1
       for (int kt = 0; kt < KT; ++kt) {
         mbar_wait(full + st, ph);
-        if (full_tile) mma_ktile_kmajor_rows<8>(acc, As + st * kGBK * kLdT, Bs + st * kGBK * kLdT, fm);
+        if (full_tile) mma_ktile_kmajor_frag<8, 4>(acc, As + st * kGBK * kLdT, Bs + st * kGBK * kLdT, fm);
         else mma_ktile_kmajor_any(acc, As + st * kGBK * kLdT, Bs + st * kGBK * kLdT, fm);
         __syncwarp();
         if (lane == 0) mbar_arrive(empty + st);
