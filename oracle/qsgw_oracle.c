@@ -196,3 +196,59 @@ int qsgw_oracle_sigma_diag(int N, int o, int naux, int64_t n_pole, const double 
   free(V); free(w); free(accR); free(accI);
   return 0;
 }
+
+/* ---- row 8(f).3, first half: the second-order Coulomb (direct) term of the qsMP2 self-energy ----------------
+ * First sum of Eq. (20) put into Eq. (21), closed shell (the spin sum over sigma'
+ * gives a factor 2), RI integrals (mp|ia) = sum_P B[P][m][p] B[P][i][a], real part as for qsGW:
+ *   Sigma[m][n] = 1/2 * sum_i sum_a sum_p 2 [ (mp|ia)(pn|ai) Dd(i,a,p,eps[n]) + (np|ia)(pm|ai) Dd(i,a,p,eps[m]) ]
+ *   Dd(i,a,p,omega) = occ[p]     * x1/(x1^2+eta^2),  x1 = omega + eps[a] - eps[i] - eps[p]
+ *                   + (1-occ[p]) * x2/(x2^2+eta^2),  x2 = omega + eps[i] - eps[a] - eps[p]
+ * i < o <= a, p over all N states; (pn|ai) is read literally as sum_P B[P][p][n] B[P][a][i].
+ * The second sum of Eq. (20) (second-order exchange, SOX) is NOT part of this function.
+ * Sigma is N x N row-major.  Returns 0, or -1 on allocation failure / bad arguments. */
+int qsgw_oracle_mp2_direct(int N, int o, int naux, const double *B, const double *eps, const double *occ, double eta,
+                           double *Sigma) {
+  if (N < 2 || o < 1 || o >= N || naux < 1 || !(eta > 0.0)) return -1;
+  long double *acc = (long double *)malloc(sizeof(long double) * (size_t)N * N);
+  double *L = (double *)malloc(sizeof(double) * (size_t)N * N);   /* L[m][p] = (mp|ia) */
+  double *R = (double *)malloc(sizeof(double) * (size_t)N * N);   /* R[p][n] = (pn|ai) */
+  if (!acc || !L || !R) { free(acc); free(L); free(R); return -1; }
+  for (size_t k = 0; k < (size_t)N * N; ++k) acc[k] = 0.0L;
+  for (int i = 0; i < o; ++i) {
+    for (int a = o; a < N; ++a) {
+#pragma omp parallel for schedule(static)
+      for (int m = 0; m < N; ++m) {
+        for (int p = 0; p < N; ++p) {
+          double l = 0.0, r = 0.0;
+          for (int P = 0; P < naux; ++P) {
+            const double *BP = B + (size_t)P * N * N;
+            l += BP[(size_t)m * N + p] * BP[(size_t)i * N + a];
+            r += BP[(size_t)m * N + p] * BP[(size_t)a * N + i];     /* here m, p play the roles of p, n */
+          }
+          L[(size_t)m * N + p] = l;
+          R[(size_t)m * N + p] = r;
+        }
+      }
+#pragma omp parallel for schedule(static)
+      for (int m = 0; m < N; ++m) {
+        for (int n = 0; n < N; ++n) {
+          double t = 0.0;
+          for (int p = 0; p < N; ++p) {
+            /* <m|Sigma(eps_n)|n> uses (mp|ia)(pn|ai); <n|Sigma(eps_m)|m> uses (np|ia)(pm|ai)   (Eq. (21)) */
+            const double om[2] = {eps[n], eps[m]};
+            const double num[2] = {L[(size_t)m * N + p] * R[(size_t)p * N + n], L[(size_t)n * N + p] * R[(size_t)p * N + m]};
+            for (int k = 0; k < 2; ++k) {
+              const double x1 = om[k] + eps[a] - eps[i] - eps[p];
+              const double x2 = om[k] + eps[i] - eps[a] - eps[p];
+              t += 2.0 * num[k] * (occ[p] * (x1 / (x1 * x1 + eta * eta)) + (1.0 - occ[p]) * (x2 / (x2 * x2 + eta * eta)));
+            }
+          }
+          acc[(size_t)m * N + n] += 0.5L * (long double)t;
+        }
+      }
+    }
+  }
+  for (size_t k = 0; k < (size_t)N * N; ++k) Sigma[k] = (double)acc[k];
+  free(acc); free(L); free(R);
+  return 0;
+}

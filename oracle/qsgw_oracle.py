@@ -53,6 +53,8 @@ def _load():
         lib.qsgw_oracle_sigma_diag.restype = ctypes.c_int
         lib.qsgw_oracle_sigma_diag.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i64, dp, dp, dp, dp, dp, i64,
                                                ctypes.c_double, ctypes.c_int, dp, ctypes.c_int, ip, dp, dp]
+        lib.qsgw_oracle_mp2_direct.restype = ctypes.c_int
+        lib.qsgw_oracle_mp2_direct.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, ctypes.c_double, dp]
         _lib = lib
     return _lib
 
@@ -180,3 +182,19 @@ def ao_to_mo(B_ao, C):
     if B_ao.ndim != 3 or B_ao.shape[1] != B_ao.shape[2] or C.ndim != 2 or C.shape[0] != B_ao.shape[1]:
         raise ValueError("need B_ao [naux, nao, nao] and C [nao, n_mo]")
     return np.matmul(C.T[None, :, :], np.matmul(B_ao, C[None, :, :]))
+
+
+def mp2_direct(B, eps, occ, eta: float, n_occ: int):
+    """Second-order Coulomb (direct) term of the qsMP2 self-energy: first sum of Eq. (20) in Eq. (21), closed shell
+    (PAPER.md:174-186).  The SOX term is not included.  Returns Sigma [N, N]."""
+    B = _f64(B)
+    naux, N, N2 = B.shape
+    if N != N2:
+        raise ValueError("B must be [naux, N, N]")
+    eps = _f64(eps, (N,))
+    occ = _f64(occ, (N,))
+    out = np.empty((N, N))
+    rc = _load().qsgw_oracle_mp2_direct(N, n_occ, naux, _dp(B), _dp(eps), _dp(occ), float(eta), _dp(out))
+    if rc != 0:
+        raise RuntimeError(f"qsgw_oracle_mp2_direct failed with {rc}")
+    return out
