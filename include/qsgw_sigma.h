@@ -141,6 +141,19 @@ int qsgw_sigma_diag_build(qsgw_sigma_plan *plan, const double *B, const double *
                           const double *omega_grid, int n_omega, double *SigmaRe, double *SigmaIm);
 
 /*
+ * Row 8(f).3, first half: the second-order Coulomb (direct) term of the qsMP2 self-energy -- the first sum of Eq. (20)
+ * put into Eq. (21), closed shell, RI integrals, real part:
+ *   Sigma[m][n] = 1/2 sum_{i<o<=a} sum_p 2 [ (mp|ia)(pn|ai) Dd(eps[n]) + (np|ia)(pm|ai) Dd(eps[m]) ],
+ *   Dd(omega) = occ[p] x1/(x1^2+eta^2) + (1-occ[p]) x2/(x2^2+eta^2),  x1 = omega + eps[a]-eps[i] - eps[p],  x2 = omega - (eps[a]-eps[i]) - eps[p].
+ * This is Eq. (17)-(19) with the (ia) pairs as poles, X+Y = 1 and Omega_ia = eps[a] - eps[i], so the library runs its stages 2-3
+ * on pole weights V[P][ia] = B[P][i][a] gathered chunk by chunk (no stage 1, no Z).  The second-order exchange (SOX) sum of
+ * Eq. (20) is NOT included.  B, eps, occ, eta, Sigma as in qsgw_sigma_build (B symmetric in its last two indices); the plan may
+ * have any n_pole_max.  Asynchronous on the plan's stream; a small Omega buffer is allocated on the first call (ALLOC if it fails).
+ */
+int qsgw_mp2_direct_build(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ, double eta,
+                          double *Sigma);
+
+/*
  * Row 8(f).2 of the scope table: the RI AO->MO transformation that produces the B argument of the calls above, once per
  * qsGW iteration (the RI analogue of Eq. (16); RI remark PAPER.md:120):
  *   B_mo[P][p][q] = sum_mu sum_nu C[mu][p] * C[nu][q] * B_ao[P][mu][nu]        (B_mo[P] = C^T B_ao[P] C)

@@ -43,7 +43,7 @@ struct qsgw_sigma_plan {
   // workspace
   int64_t n_pair = 0, ldp = 0, ld_aux = 0, ldv = 0, ldw = 0;
   int nsplit = 0, m_per_split = 0, ntile_1d = 0;
-  double *Bp = nullptr, *BovT = nullptr, *V = nullptr, *W = nullptr, *Tpart = nullptr;
+  double *Bp = nullptr, *BovT = nullptr, *V = nullptr, *W = nullptr, *Tpart = nullptr, *mp2_omega = nullptr;
   int2 *pairs = nullptr;
   size_t bytes = 0;
 
@@ -198,7 +198,34 @@ struct DiagArgs {
   double *Re, *Im;
 };
 
-// diag == nullptr: stage 3 of the qsGW matrix; otherwise the G0W0 diagonal kernel takes its place
+// Stages 2 and 3 for one chunk of sc <= s_chunk poles whose pole weights are the columns Vc[P][0..sc) (leading dimension
+// ldv) and whose energies are Omega_c[0..sc).  diag == nullptr: stage 3 of the qsGW matrix; otherwise the G0W0 diagonal
+// kernel takes its place.
+int run_chunk(qsgw_sigma_plan *p, const double *Vc, const double *Omega_c, int sc, const DiagArgs *diag) {
+  {  // stage 2: w[(p<=m)][s] = sqrt(2) sum_P Bp[P][(p,m)] * Vc[P][s], scattered to W[(m,p)] and W[(p,m)]
+    ScopedTimer t(p, kStage2);
+    EpiPairScatter epi{p->W, p->ldw, p->pairs, p->n_mo, std::sqrt(2.0)};
+    int rc = launch_gemm<2>(p, p->Bp, p->ldp, Vc, p->ldv, (int)p->n_pair, sc, p->n_aux, epi);
+    if (rc) return rc;
+  }
+  if (diag) {  // G0W0 diagonal: Re/Im[p][k] += sum_m sum_{s in chunk} w^2 / (omega_k - eps_m +- Omega_s -+ i eta)
+    ScopedTimer t(p, kDiag);
+    const size_t smem = sizeof(double) * ((size_t)sc + (kDiagThreads / 32) * 2 * kDiagKW);
+    sigma_diag_kernel<<<dim3(p->n_mo, (diag->n_omega + kDiagKW - 1) / kDiagKW), kDiagThreads, smem, p->stream>>>(
+        p->W, p->ldw, p->eps, p->occ, Omega_c, p->n_mo, sc, p->eta, diag->omega_grid, diag->n_omega, diag->Re, diag->Im);
+    p->kernel_launches += 1;
+    QSGW_CUDA(p, cudaGetLastError());
+  } else {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
+    ScopedTimer t(p, kStage3);
+    const int ntp = (p->n_mo + kTP - 1) / kTP, ntq = (p->n_mo + kTQ - 1) / kTQ;
+    sigma_accumulate_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
+        p->W, p->ldw, p->eps, p->occ, Omega_c, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart);
+    p->kernel_launches += 1;
+    QSGW_CUDA(p, cudaGetLastError());
+  }
+  return QSGW_SIGMA_OK;
+}
+
 int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64_t ldz, int64_t n_pole,
                  const DiagArgs *diag = nullptr) {
   if (!p->begun) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles called before begin");
@@ -213,7 +240,6 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
                                       (int)kSigmaSmemBytes));
     sigma_configured = true;
   }
-  const int ntp = (p->n_mo + kTP - 1) / kTP, ntq = (p->n_mo + kTQ - 1) / kTQ;
   for (int64_t v0 = 0; v0 < n_pole; v0 += p->v_cols) {
     const int64_t nv = std::min<int64_t>(p->v_cols, n_pole - v0);
     {  // stage 1 for all poles of this range at once (enough tiles to fill the SMs evenly):
@@ -228,27 +254,8 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
     }
     for (int64_t c0 = 0; c0 < nv; c0 += p->s_chunk) {
       const int sc = (int)std::min<int64_t>(p->s_chunk, nv - c0);
-      {  // stage 2: w[(p<=m)][s] = sqrt(2) sum_P Bp[P][(p,m)] * V[P][c0+s], scattered to W[(m,p)] and W[(p,m)]
-        ScopedTimer t(p, kStage2);
-        EpiPairScatter epi{p->W, p->ldw, p->pairs, p->n_mo, std::sqrt(2.0)};
-        int rc = launch_gemm<2>(p, p->Bp, p->ldp, p->V + c0, p->ldv, (int)p->n_pair, sc, p->n_aux, epi);
-        if (rc) return rc;
-      }
-      if (diag) {  // G0W0 diagonal: Re/Im[p][k] += sum_m sum_{s in chunk} w^2 / (omega_k - eps_m +- Omega_s -+ i eta)
-        ScopedTimer t(p, kDiag);
-        const size_t smem = sizeof(double) * ((size_t)sc + (kDiagThreads / 32) * 2 * kDiagKW);
-        sigma_diag_kernel<<<dim3(p->n_mo, (diag->n_omega + kDiagKW - 1) / kDiagKW), kDiagThreads, smem, p->stream>>>(
-            p->W, p->ldw, p->eps, p->occ, Omega + v0 + c0, p->n_mo, sc, p->eta, diag->omega_grid, diag->n_omega,
-            diag->Re, diag->Im);
-        p->kernel_launches += 1;
-        QSGW_CUDA(p, cudaGetLastError());
-      } else {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
-        ScopedTimer t(p, kStage3);
-        sigma_accumulate_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
-            p->W, p->ldw, p->eps, p->occ, Omega + v0 + c0, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart);
-        p->kernel_launches += 1;
-        QSGW_CUDA(p, cudaGetLastError());
-      }
+      int rc = run_chunk(p, p->V + c0, Omega + v0 + c0, sc, diag);
+      if (rc) return rc;
     }
   }
   p->poles += n_pole;
@@ -476,6 +483,35 @@ int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps
   return QSGW_SIGMA_OK;
 }
 
+int qsgw_mp2_direct_build(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, double eta,
+                          double *Sigma) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  if (!Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "mp2_direct_build: Sigma must be non-NULL");
+  if (!p->mp2_omega && (rc = dev_alloc(p, &p->mp2_omega, (size_t)p->ldw, "orbital-energy differences of a chunk"))) return rc;
+  static bool sigma_configured = false;
+  if (!sigma_configured) {
+    QSGW_CUDA(p, cudaFuncSetAttribute(sigma_accumulate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)kSigmaSmemBytes));
+    sigma_configured = true;
+  }
+  if ((rc = do_begin(p, B, eps, occ, eta))) return rc;
+  // the (ia) pairs play the role of the poles: V[P][ia] = B[P][i][a] (X+Y = 1), Omega_ia = eps_a - eps_i
+  for (int64_t s0 = 0; s0 < p->n_ov; s0 += p->s_chunk) {
+    const int sc = (int)std::min<int64_t>(p->s_chunk, p->n_ov - s0);
+    {
+      ScopedTimer t(p, kPack);
+      mp2_chunk_kernel<<<dim3((sc + 255) / 256, p->n_aux + 1), 256, 0, p->stream>>>(B, eps, p->n_mo, p->n_occ, p->n_aux, s0, sc,
+                                                                                  p->V, p->ldv, p->mp2_omega);
+      p->kernel_launches += 1;
+      QSGW_CUDA(p, cudaGetLastError());
+    }
+    if ((rc = run_chunk(p, p->V, p->mp2_omega, sc, nullptr))) { p->begun = false; return rc; }
+  }
+  p->poles += p->n_ov;
+  return do_finish(p, Sigma);
+}
+
 size_t qsgw_ri_ao_to_mo_work_doubles(int n_aux, int n_ao, int n_mo) {
   if (n_aux < 1 || n_ao < 1 || n_mo < 1) return 0;
   return (size_t)n_aux * (size_t)n_ao * (size_t)round_up(n_mo, 2);
@@ -533,7 +569,7 @@ int qsgw_sigma_destroy(qsgw_sigma_plan *p) {
     cudaFree(p->hOmega[b]); cudaFree(p->hZ[b]);
   }
   cudaFree(p->hB); cudaFree(p->hEps); cudaFree(p->hOcc); cudaFree(p->hSigma);
-  cudaFree(p->Bp); cudaFree(p->BovT); cudaFree(p->V); cudaFree(p->W); cudaFree(p->Tpart); cudaFree(p->pairs);
+  cudaFree(p->Bp); cudaFree(p->BovT); cudaFree(p->V); cudaFree(p->W); cudaFree(p->Tpart); cudaFree(p->pairs); cudaFree(p->mp2_omega);
   cudaGetLastError();
   delete p;
   return QSGW_SIGMA_OK;

@@ -50,6 +50,20 @@ __global__ void pack_ov_transposed_kernel(const double *__restrict__ B, int n_mo
   }
 }
 
+// Row 8(f).3 (direct term of qsMP2): the (ia) pairs s = i*v + (a-o) take the place of the poles.  blockIdx.y < n_aux:
+// V[P][s - s0] = B[P][i][a] (the residues (mp|ia) are then w with X+Y = 1); blockIdx.y == n_aux: Omega[s - s0] = eps_a - eps_i.
+__global__ void mp2_chunk_kernel(const double *__restrict__ B, const double *__restrict__ eps, int n_mo, int n_occ, int n_aux,
+                                 int64_t s0, int sc, double *__restrict__ V, int64_t ldv, double *__restrict__ Omega) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= sc) return;
+  const int v = n_mo - n_occ;
+  const int64_t s = s0 + j;
+  const int i = (int)(s / v), a = n_occ + (int)(s - (int64_t)i * v);
+  const int P = blockIdx.y;
+  if (P < n_aux) V[(int64_t)P * ldv + j] = B[((int64_t)P * n_mo + i) * n_mo + a];
+  else Omega[j] = eps[a] - eps[i];
+}
+
 // ---------------------------------------------------------------- stage 3
 // D(m,s,omega) = occ_m * x1/(x1^2+eta^2) + (1-occ_m) * x2/(x2^2+eta^2),  x1 = (omega-eps_m)+Omega_s,
 // x2 = (omega-eps_m)-Omega_s: real part of the two terms of Eq. (17).  d = omega - eps_m.
