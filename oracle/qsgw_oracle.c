@@ -39,6 +39,11 @@
  * Python-complex evaluation of Eq. (17) through the non-RI 4-index form, Re Sigma_pp(eps_p) == diagonal of the
  * (separately pinned) qsGW matrix, exact power-of-two scaling, additivity over poles, sign of Im, eta -> 0 limit.
  *
+ * Further rows at the end of this file: qsgw_oracle_mp2_direct and qsgw_oracle_mp2 (Eqs. (20)-(21), PAPER.md:174-186;
+ * pins in tests/test_oracle_mp2_pins.py: the hand-solved two-state rationals, a literal complex spin-orbital brute force
+ * of both sums incl. unsymmetric B, identity with the GW oracle at Z = 1, SOX = -direct/2 for rank-one B).  The RI AO->MO
+ * transformation (oracle.ao_to_mo) lives in qsgw_oracle.py as a numpy matmul; pins in tests/test_oracle_aomo_pins.py.
+ *
  * Floating point: products and the P-, ia- and m-sums are plain double; the running sum
  * over poles s of step 3 is kept in long double so that the oracle's own rounding is far
  * below the 1e-9 parity budget.
@@ -250,5 +255,62 @@ int qsgw_oracle_mp2_direct(int N, int o, int naux, const double *B, const double
   }
   for (size_t k = 0; k < (size_t)N * N; ++k) Sigma[k] = (double)acc[k];
   free(acc); free(L); free(R);
+  return 0;
+}
+
+/* ---- row 8(f).3, whole: the qsMP2 correlation self-energy, direct + second-order exchange (SOX) ------------------
+ * Both sums of Eq. (20) put into Eq. (21), closed shell: the direct sum runs over both
+ * spins sigma' (factor 2), the SOX sum over the same spin only (factor 1, sign -), RI integrals, real part:
+ *   Sigma[m][n] = 1/2 sum_i sum_a sum_p ( [2 (mp|ia)(pn|ai) - (mp|ia)(pi|an)] Dd(i,a,p,eps[n])
+ *                                       + [2 (np|ia)(pm|ai) - (np|ia)(pi|am)] Dd(i,a,p,eps[m]) )
+ * with Dd as in qsgw_oracle_mp2_direct; every integral is read literally, (xy|zw) = sum_P B[P][x][y] B[P][z][w].
+ * sox_only != 0 drops the direct part.  Returns 0 / -1 as above. */
+int qsgw_oracle_mp2(int N, int o, int naux, const double *B, const double *eps, const double *occ, double eta,
+                    int sox_only, double *Sigma) {
+  if (N < 2 || o < 1 || o >= N || naux < 1 || !(eta > 0.0)) return -1;
+  const size_t NN = (size_t)N * N;
+  long double *acc = (long double *)malloc(sizeof(long double) * NN);
+  double *L = (double *)malloc(sizeof(double) * NN);    /* L[x][y]  = (xy|ia) */
+  double *R = (double *)malloc(sizeof(double) * NN);    /* R[x][y]  = (xy|ai) */
+  double *E = (double *)malloc(sizeof(double) * NN);    /* E[p][n]  = (pi|an) */
+  if (!acc || !L || !R || !E) { free(acc); free(L); free(R); free(E); return -1; }
+  for (size_t k = 0; k < NN; ++k) acc[k] = 0.0L;
+  const double cd = sox_only ? 0.0 : 2.0;
+  for (int i = 0; i < o; ++i) {
+    for (int a = o; a < N; ++a) {
+#pragma omp parallel for schedule(static)
+      for (int x = 0; x < N; ++x) {
+        for (int y = 0; y < N; ++y) {
+          double l = 0.0, r = 0.0, e = 0.0;
+          for (int P = 0; P < naux; ++P) {
+            const double *BP = B + (size_t)P * NN;
+            l += BP[(size_t)x * N + y] * BP[(size_t)i * N + a];
+            r += BP[(size_t)x * N + y] * BP[(size_t)a * N + i];
+            e += BP[(size_t)x * N + i] * BP[(size_t)a * N + y];
+          }
+          L[(size_t)x * N + y] = l; R[(size_t)x * N + y] = r; E[(size_t)x * N + y] = e;
+        }
+      }
+#pragma omp parallel for schedule(static)
+      for (int m = 0; m < N; ++m) {
+        for (int n = 0; n < N; ++n) {
+          double t = 0.0;
+          for (int p = 0; p < N; ++p) {
+            const double om[2] = {eps[n], eps[m]};
+            const double num[2] = {L[(size_t)m * N + p] * (cd * R[(size_t)p * N + n] - E[(size_t)p * N + n]),
+                                   L[(size_t)n * N + p] * (cd * R[(size_t)p * N + m] - E[(size_t)p * N + m])};
+            for (int k = 0; k < 2; ++k) {
+              const double x1 = om[k] + eps[a] - eps[i] - eps[p];
+              const double x2 = om[k] + eps[i] - eps[a] - eps[p];
+              t += num[k] * (occ[p] * (x1 / (x1 * x1 + eta * eta)) + (1.0 - occ[p]) * (x2 / (x2 * x2 + eta * eta)));
+            }
+          }
+          acc[(size_t)m * N + n] += 0.5L * (long double)t;
+        }
+      }
+    }
+  }
+  for (size_t k = 0; k < NN; ++k) Sigma[k] = (double)acc[k];
+  free(acc); free(L); free(R); free(E);
   return 0;
 }

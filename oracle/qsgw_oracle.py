@@ -55,6 +55,8 @@ def _load():
                                                ctypes.c_double, ctypes.c_int, dp, ctypes.c_int, ip, dp, dp]
         lib.qsgw_oracle_mp2_direct.restype = ctypes.c_int
         lib.qsgw_oracle_mp2_direct.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, ctypes.c_double, dp]
+        lib.qsgw_oracle_mp2.restype = ctypes.c_int
+        lib.qsgw_oracle_mp2.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, ctypes.c_double, ctypes.c_int, dp]
         _lib = lib
     return _lib
 
@@ -197,4 +199,20 @@ def mp2_direct(B, eps, occ, eta: float, n_occ: int):
     rc = _load().qsgw_oracle_mp2_direct(N, n_occ, naux, _dp(B), _dp(eps), _dp(occ), float(eta), _dp(out))
     if rc != 0:
         raise RuntimeError(f"qsgw_oracle_mp2_direct failed with {rc}")
+    return out
+
+
+def mp2(B, eps, occ, eta: float, n_occ: int, sox_only: bool = False):
+    """qsMP2 correlation self-energy: both sums of Eq. (20) (direct and second-order exchange) in Eq. (21), closed
+    shell.  ``sox_only`` returns the exchange part alone.  Returns Sigma [N, N]."""
+    B = _f64(B)
+    naux, N, N2 = B.shape
+    if N != N2:
+        raise ValueError("B must be [naux, N, N]")
+    eps = _f64(eps, (N,))
+    occ = _f64(occ, (N,))
+    out = np.empty((N, N))
+    rc = _load().qsgw_oracle_mp2(N, n_occ, naux, _dp(B), _dp(eps), _dp(occ), float(eta), 1 if sox_only else 0, _dp(out))
+    if rc != 0:
+        raise RuntimeError(f"qsgw_oracle_mp2 failed with {rc}")
     return out

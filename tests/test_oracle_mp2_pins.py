@@ -76,3 +76,54 @@ def test_equals_the_gw_expression_with_unit_z_and_orbital_energy_differences():
     got = oracle.mp2_direct(B, eps, occ, 1e-3, o)
     assert np.max(np.abs(got - want)) <= 1e-12 * np.abs(want).max()
     assert np.max(np.abs(got - got.T)) <= 1e-13 * np.abs(got).max()
+
+
+# ---------------------------------------------------------------- whole qsMP2: direct + second-order exchange
+def _bruteforce_spin_orbital(B, eps, occ, eta, o):
+    """Eq. (20) in spin orbitals, both sums literally: the direct sum runs over sigma' in {up, down}, the SOX sum has all
+    spins equal; 4-index integrals (xy|zw) = sum_P B_xy B_zw; complex denominators; Eq. (21); real part."""
+    naux, N, _ = B.shape
+    eri = np.einsum("Pxy,Pzw->xyzw", B, B)
+    def den(w, i, a, p):
+        return (occ[p] / complex(w + eps[a] - eps[i] - eps[p], -eta)
+                + (1.0 - occ[p]) / complex(w + eps[i] - eps[a] - eps[p], +eta))
+    def sigma_w(m, n, w):
+        tot = 0.0 + 0.0j
+        for i in range(o):
+            for a in range(o, N):
+                for p in range(N):
+                    d = den(w, i, a, p)
+                    for spin in range(2):
+                        tot += eri[m, p, i, a] * eri[p, n, a, i] * d          # direct, sigma' = spin
+                    tot -= eri[m, p, i, a] * eri[p, i, a, n] * d              # SOX, one spin
+        return tot
+    out = np.zeros((N, N))
+    for m in range(N):
+        for n in range(N):
+            out[m, n] = 0.5 * (sigma_w(m, n, eps[n]) + sigma_w(n, m, eps[m])).real
+    return out
+
+
+@pytest.mark.parametrize("N,o,naux,seed,sym", [(4, 1, 3, 1, True), (5, 2, 2, 2, True), (5, 3, 3, 3, False)])
+def test_literal_eq20_both_sums(N, o, naux, seed, sym):
+    rng = np.random.default_rng(seed)
+    B, eps, occ = _case(rng, N, o, naux, sym)
+    want = _bruteforce_spin_orbital(B, eps, occ, 0.05, o)
+    got = oracle.mp2(B, eps, occ, 0.05, o)
+    assert np.max(np.abs(got - want)) <= 1e-12 * np.abs(want).max()
+    # the parts add up, and the direct part is the function pinned above
+    sox = oracle.mp2(B, eps, occ, 0.05, o, sox_only=True)
+    assert np.max(np.abs(oracle.mp2_direct(B, eps, occ, 0.05, o) + sox - got)) <= 1e-13 * np.abs(got).max()
+
+
+def test_one_auxiliary_function_sox_is_minus_half_the_direct_term():
+    """naux = 1: (mp|ia)(pi|an) = B_mp B_ia B_pi B_an and (mp|ia)(pn|ai) = B_mp B_ia B_pn B_ai; no general relation, but
+    with a rank-one B = u u^T every 4-index integral factorises, (xy|zw) = u_x u_y u_z u_w, so SOX = -1/2 direct exactly."""
+    rng = np.random.default_rng(8)
+    N, o = 6, 2
+    u = rng.normal(0, 1, N)
+    B = np.outer(u, u)[None, :, :]
+    _, eps, occ = _case(rng, N, o, 1)
+    d = oracle.mp2_direct(B, eps, occ, 0.01, o)
+    sox = oracle.mp2(B, eps, occ, 0.01, o, sox_only=True)
+    assert np.max(np.abs(sox + 0.5 * d)) <= 1e-13 * np.abs(d).max()
