@@ -147,11 +147,23 @@ int qsgw_sigma_diag_build(qsgw_sigma_plan *plan, const double *B, const double *
  *   Dd(omega) = occ[p] x1/(x1^2+eta^2) + (1-occ[p]) x2/(x2^2+eta^2),  x1 = omega + eps[a]-eps[i] - eps[p],  x2 = omega - (eps[a]-eps[i]) - eps[p].
  * This is Eq. (17)-(19) with the (ia) pairs as poles, X+Y = 1 and Omega_ia = eps[a] - eps[i], so the library runs its stages 2-3
  * on pole weights V[P][ia] = B[P][i][a] gathered chunk by chunk (no stage 1, no Z).  The second-order exchange (SOX) sum of
- * Eq. (20) is NOT included.  B, eps, occ, eta, Sigma as in qsgw_sigma_build (B symmetric in its last two indices); the plan may
+ * Eq. (20) is NOT included here (qsgw_mp2_build adds it).  B, eps, occ, eta, Sigma as in qsgw_sigma_build (B symmetric in its last two indices); the plan may
  * have any n_pole_max.  Asynchronous on the plan's stream; a small Omega buffer is allocated on the first call (ALLOC if it fails).
  */
 int qsgw_mp2_direct_build(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ, double eta,
                           double *Sigma);
+
+/*
+ * Row 8(f).3, whole: the qsMP2 correlation self-energy, both sums of Eq. (20) in Eq. (21), closed shell:
+ *   Sigma[m][n] = 1/2 sum_{i<o<=a} sum_p ( [2 (mp|ia)(pn|ai) - (mp|ia)(pi|an)] Dd(eps[n]) + [2 (np|ia)(pm|ai) - (np|ia)(pi|am)] Dd(eps[m]) )
+ * The direct sum is computed as in qsgw_mp2_direct_build.  The second-order exchange (SOX) sum runs, for every occupied i,
+ * one batched GEMM for the exchange integrals (pi|an), stage 2 for -(mp|ia) and the fused D-scaling + contraction kernel of
+ * stage 3 with those two as its left and right operands (virtual a as the "poles", p as the internal state); everything
+ * accumulates into the same split-K partial tiles and one epilogue symmetrises.  O(o N^2 (N + v) naux + o v N^3) flops.
+ * Arguments as qsgw_mp2_direct_build; B must be symmetric in its last two indices.  A buffer of n_mo^3 doubles for the
+ * exchange integrals of one i is allocated on the first call (ALLOC if it does not fit).
+ */
+int qsgw_mp2_build(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ, double eta, double *Sigma);
 
 /*
  * Row 8(f).2 of the scope table: the RI AO->MO transformation that produces the B argument of the calls above, once per

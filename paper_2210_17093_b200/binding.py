@@ -22,7 +22,7 @@ QSGW_SIGMA_ERR_CUDA = -3
 
 EXPORTS = (
     "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
-    "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_mp2_direct_build", "qsgw_ri_ao_to_mo", "qsgw_ri_ao_to_mo_work_doubles", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
+    "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_mp2_direct_build", "qsgw_mp2_build", "qsgw_ri_ao_to_mo", "qsgw_ri_ao_to_mo_work_doubles", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
     "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_copy_workspace", "qsgw_sigma_version", "qsgw_sigma_fp64_probe",
 )
 
@@ -77,6 +77,8 @@ def load_library() -> ctypes.CDLL:
         lib.qsgw_sigma_diag_build.argtypes = [vp, dp, dp, dp, dp, dp, i64, i64, cd, dp, ci, dp, dp]
         lib.qsgw_mp2_direct_build.restype = ci
         lib.qsgw_mp2_direct_build.argtypes = [vp, dp, dp, dp, cd, dp]
+        lib.qsgw_mp2_build.restype = ci
+        lib.qsgw_mp2_build.argtypes = [vp, dp, dp, dp, cd, dp]
         lib.qsgw_ri_ao_to_mo.restype = ci
         lib.qsgw_ri_ao_to_mo.argtypes = [dp, dp, ci, ci, ci, dp, dp, vp]
         lib.qsgw_ri_ao_to_mo_work_doubles.restype = ctypes.c_size_t
@@ -237,6 +239,19 @@ def qsgw_mp2_direct_build(plan: Plan, B, eps, occ, eta: float, Sigma: Optional[t
         Sigma = torch.empty((N, N), dtype=torch.float64, device=B.device)
     rc = load_library().qsgw_mp2_direct_build(plan.handle, _dev(B, "B", (plan.n_aux, N, N)), _dev(eps, "eps", (N,)),
                                               _dev(occ, "occ", (N,)), float(eta), _dev(Sigma, "Sigma", (N, N)))
+    _check(rc, plan.handle)
+    return Sigma
+
+
+def qsgw_mp2_build(plan: Plan, B, eps, occ, eta: float, Sigma: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """qsMP2 correlation self-energy: direct + second-order exchange sums of Eq. (20) in Eq. (21)."""
+    N = plan.n_mo
+    if not B.is_contiguous() or not eps.is_contiguous() or not occ.is_contiguous():
+        raise ValueError("B, eps, occ must be contiguous")
+    if Sigma is None:
+        Sigma = torch.empty((N, N), dtype=torch.float64, device=B.device)
+    rc = load_library().qsgw_mp2_build(plan.handle, _dev(B, "B", (plan.n_aux, N, N)), _dev(eps, "eps", (N,)),
+                                       _dev(occ, "occ", (N,)), float(eta), _dev(Sigma, "Sigma", (N, N)))
     _check(rc, plan.handle)
     return Sigma
 

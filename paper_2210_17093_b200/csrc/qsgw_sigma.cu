@@ -43,7 +43,7 @@ struct qsgw_sigma_plan {
   // workspace
   int64_t n_pair = 0, ldp = 0, ld_aux = 0, ldv = 0, ldw = 0;
   int nsplit = 0, m_per_split = 0, ntile_1d = 0;
-  double *Bp = nullptr, *BovT = nullptr, *V = nullptr, *W = nullptr, *Tpart = nullptr, *mp2_omega = nullptr;
+  double *Bp = nullptr, *BovT = nullptr, *V = nullptr, *W = nullptr, *Tpart = nullptr, *mp2_omega = nullptr, *mp2_y = nullptr;
   int2 *pairs = nullptr;
   size_t bytes = 0;
 
@@ -198,16 +198,36 @@ struct DiagArgs {
   double *Re, *Im;
 };
 
+// Stage 2 for one chunk: W[(m,p)][s] = W[(p,m)][s] = alpha * sum_P Bp[P][(p,m)] * Vc[P][s], s < sc (leading dimension ldv)
+int run_stage2(qsgw_sigma_plan *p, const double *Vc, int sc, double alpha) {
+  ScopedTimer t(p, kStage2);
+  EpiPairScatter epi{p->W, p->ldw, p->pairs, p->n_mo, alpha};
+  return launch_gemm<2>(p, p->Bp, p->ldp, Vc, p->ldv, (int)p->n_pair, sc, p->n_aux, epi);
+}
+
+// Stage 3 for one chunk: Tpart[z] += (WA.D) WB^T over the internal states of split z and the chunk's sc poles
+int run_stage3(qsgw_sigma_plan *p, const double *WA, int64_t ldA, const double *WB, int64_t ldB, const double *Omega_c, int sc) {
+  static bool configured = false;
+  if (!configured) {
+    QSGW_CUDA(p, cudaFuncSetAttribute(sigma_accumulate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)kSigmaSmemBytes));
+    configured = true;
+  }
+  ScopedTimer t(p, kStage3);
+  const int ntp = (p->n_mo + kTP - 1) / kTP, ntq = (p->n_mo + kTQ - 1) / kTQ;
+  sigma_accumulate_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
+      WA, ldA, WB, ldB, p->eps, p->occ, Omega_c, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart);
+  p->kernel_launches += 1;
+  QSGW_CUDA(p, cudaGetLastError());
+  return QSGW_SIGMA_OK;
+}
+
 // Stages 2 and 3 for one chunk of sc <= s_chunk poles whose pole weights are the columns Vc[P][0..sc) (leading dimension
 // ldv) and whose energies are Omega_c[0..sc).  diag == nullptr: stage 3 of the qsGW matrix; otherwise the G0W0 diagonal
 // kernel takes its place.
 int run_chunk(qsgw_sigma_plan *p, const double *Vc, const double *Omega_c, int sc, const DiagArgs *diag) {
-  {  // stage 2: w[(p<=m)][s] = sqrt(2) sum_P Bp[P][(p,m)] * Vc[P][s], scattered to W[(m,p)] and W[(p,m)]
-    ScopedTimer t(p, kStage2);
-    EpiPairScatter epi{p->W, p->ldw, p->pairs, p->n_mo, std::sqrt(2.0)};
-    int rc = launch_gemm<2>(p, p->Bp, p->ldp, Vc, p->ldv, (int)p->n_pair, sc, p->n_aux, epi);
-    if (rc) return rc;
-  }
+  int rc = run_stage2(p, Vc, sc, std::sqrt(2.0));
+  if (rc) return rc;
   if (diag) {  // G0W0 diagonal: Re/Im[p][k] += sum_m sum_{s in chunk} w^2 / (omega_k - eps_m +- Omega_s -+ i eta)
     ScopedTimer t(p, kDiag);
     const size_t smem = sizeof(double) * ((size_t)sc + (kDiagThreads / 32) * 2 * kDiagKW);
@@ -215,15 +235,9 @@ int run_chunk(qsgw_sigma_plan *p, const double *Vc, const double *Omega_c, int s
         p->W, p->ldw, p->eps, p->occ, Omega_c, p->n_mo, sc, p->eta, diag->omega_grid, diag->n_omega, diag->Re, diag->Im);
     p->kernel_launches += 1;
     QSGW_CUDA(p, cudaGetLastError());
-  } else {  // stage 3: Tpart[z] += (w.D) w^T over m in split z and the chunk's poles
-    ScopedTimer t(p, kStage3);
-    const int ntp = (p->n_mo + kTP - 1) / kTP, ntq = (p->n_mo + kTQ - 1) / kTQ;
-    sigma_accumulate_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
-        p->W, p->ldw, p->eps, p->occ, Omega_c, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart);
-    p->kernel_launches += 1;
-    QSGW_CUDA(p, cudaGetLastError());
+    return QSGW_SIGMA_OK;
   }
-  return QSGW_SIGMA_OK;
+  return run_stage3(p, p->W, p->ldw, p->W, p->ldw, Omega_c, sc);
 }
 
 int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64_t ldz, int64_t n_pole,
@@ -234,12 +248,6 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
     return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles: n_pole must be in [1, n_pole_max]");
   if (ldz < n_pole) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles: ldz < n_pole");
 
-  static bool sigma_configured = false;
-  if (!sigma_configured) {
-    QSGW_CUDA(p, cudaFuncSetAttribute(sigma_accumulate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)kSigmaSmemBytes));
-    sigma_configured = true;
-  }
   for (int64_t v0 = 0; v0 < n_pole; v0 += p->v_cols) {
     const int64_t nv = std::min<int64_t>(p->v_cols, n_pole - v0);
     {  // stage 1 for all poles of this range at once (enough tiles to fill the SMs evenly):
@@ -259,6 +267,66 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
     }
   }
   p->poles += n_pole;
+  return QSGW_SIGMA_OK;
+}
+
+// qsMP2, direct term: the (ia) pairs play the role of the poles, V[P][ia] = B[P][i][a] (X+Y = 1), Omega_ia = eps_a - eps_i
+int mp2_direct_chunks(qsgw_sigma_plan *p) {
+  int rc;
+  if (!p->mp2_omega && (rc = dev_alloc(p, &p->mp2_omega, (size_t)p->ldw, "orbital-energy differences of a chunk"))) return rc;
+  for (int64_t s0 = 0; s0 < p->n_ov; s0 += p->s_chunk) {
+    const int sc = (int)std::min<int64_t>(p->s_chunk, p->n_ov - s0);
+    {
+      ScopedTimer t(p, kPack);
+      mp2_chunk_kernel<<<dim3((sc + 255) / 256, p->n_aux + 1), 256, 0, p->stream>>>(p->B, p->eps, p->n_mo, p->n_occ, p->n_aux,
+                                                                                  s0, sc, p->V, p->ldv, p->mp2_omega);
+      p->kernel_launches += 1;
+      QSGW_CUDA(p, cudaGetLastError());
+    }
+    if ((rc = run_chunk(p, p->V, p->mp2_omega, sc, nullptr))) return rc;
+  }
+  p->poles += p->n_ov;
+  return QSGW_SIGMA_OK;
+}
+
+// qsMP2, second-order exchange term: -sum_{i,a,p} (mp|ia)(pi|an) Dd.  For every occupied i, with the virtual a as "poles"
+// (Omega_a = eps_a - eps_i) and p as the internal state:
+//   right operand  X[p][m][a] = -(mp|ia)  = stage 2 with V[P][a] = B[P][i][a] and alpha = -1 (one spin: no sqrt(2))
+//   left operand   Y[p][n][a] =  (pi|an)  = sum_Q B[Q][i][p] * B[Q][n][a]: one batched GEMM over n (rows p, columns a)
+//   stage 3        T[n][m] += sum_{p,a} ( Y[p][n][a] D(eps_n) ) X[p][m][a]   = Sigma^SOX_mn(eps_n); the epilogue's
+//                  (T + T^T)/2 is Eq. (21).  B symmetric in its last two indices is used (B[Q][p][i] = B[Q][i][p]).
+int mp2_sox_chunks(qsgw_sigma_plan *p) {
+  int rc;
+  const int N = p->n_mo, o = p->n_occ;
+  const int64_t ldy = round_up(N, 2), NN = (int64_t)N * N;
+  if (!p->mp2_omega && (rc = dev_alloc(p, &p->mp2_omega, (size_t)p->ldw, "orbital-energy differences of a chunk"))) return rc;
+  if (!p->mp2_y && (rc = dev_alloc(p, &p->mp2_y, (size_t)N * N * ldy, "exchange integrals (pi|an) of one i"))) return rc;
+  const int a_lo = o & ~1;                       // even start: the operands of stage 3 stay 16-byte aligned
+  const int ncol = N - a_lo;
+  const bool vB = aligned16(p->B, N);            // B + i*N (+ n*N + a_lo) 16-byte aligned for every i, n
+  for (int i = 0; i < o; ++i) {
+    {  // Y[p][n][a] for a >= a_lo: batch n, A = B[.][i][.] (k = Q, m = p, lda = N^2), Bm = B[.][n][a_lo..] (ldb = N^2)
+      ScopedTimer t(p, kStage2);
+      EpiStore epi{p->mp2_y + a_lo, (int64_t)N * ldy, 1.0, ldy, 1};
+      const double *A = p->B + (int64_t)i * N, *Bm = p->B + a_lo;
+      rc = vB ? launch_gemm_on<2, 2>(p, p->stream, p->num_sms, A, NN, Bm, NN, N, ncol, p->n_aux, epi, N, 0, N)
+              : launch_gemm_on<1, 1>(p, p->stream, p->num_sms, A, NN, Bm, NN, N, ncol, p->n_aux, epi, N, 0, N);
+      if (rc) return rc;
+      p->kernel_launches += 1;
+    }
+    for (int a0 = a_lo; a0 < N; a0 += p->s_chunk) {
+      const int sc = std::min(p->s_chunk, N - a0);
+      {
+        ScopedTimer t(p, kPack);
+        mp2_sox_chunk_kernel<<<dim3((sc + 255) / 256, p->n_aux + 1), 256, 0, p->stream>>>(
+            p->B, p->eps, N, o, p->n_aux, i, a0, sc, p->V, p->ldv, p->mp2_omega);
+        p->kernel_launches += 1;
+        QSGW_CUDA(p, cudaGetLastError());
+      }
+      if ((rc = run_stage2(p, p->V, sc, -1.0))) return rc;
+      if ((rc = run_stage3(p, p->mp2_y + a0, ldy, p->W, p->ldw, p->mp2_omega, sc))) return rc;
+    }
+  }
   return QSGW_SIGMA_OK;
 }
 
@@ -488,27 +556,18 @@ int qsgw_mp2_direct_build(qsgw_sigma_plan *p, const double *B, const double *eps
   int rc = check_plan(p);
   if (rc) return rc;
   if (!Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "mp2_direct_build: Sigma must be non-NULL");
-  if (!p->mp2_omega && (rc = dev_alloc(p, &p->mp2_omega, (size_t)p->ldw, "orbital-energy differences of a chunk"))) return rc;
-  static bool sigma_configured = false;
-  if (!sigma_configured) {
-    QSGW_CUDA(p, cudaFuncSetAttribute(sigma_accumulate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)kSigmaSmemBytes));
-    sigma_configured = true;
-  }
   if ((rc = do_begin(p, B, eps, occ, eta))) return rc;
-  // the (ia) pairs play the role of the poles: V[P][ia] = B[P][i][a] (X+Y = 1), Omega_ia = eps_a - eps_i
-  for (int64_t s0 = 0; s0 < p->n_ov; s0 += p->s_chunk) {
-    const int sc = (int)std::min<int64_t>(p->s_chunk, p->n_ov - s0);
-    {
-      ScopedTimer t(p, kPack);
-      mp2_chunk_kernel<<<dim3((sc + 255) / 256, p->n_aux + 1), 256, 0, p->stream>>>(B, eps, p->n_mo, p->n_occ, p->n_aux, s0, sc,
-                                                                                  p->V, p->ldv, p->mp2_omega);
-      p->kernel_launches += 1;
-      QSGW_CUDA(p, cudaGetLastError());
-    }
-    if ((rc = run_chunk(p, p->V, p->mp2_omega, sc, nullptr))) { p->begun = false; return rc; }
-  }
-  p->poles += p->n_ov;
+  if ((rc = mp2_direct_chunks(p))) { p->begun = false; return rc; }
+  return do_finish(p, Sigma);
+}
+
+int qsgw_mp2_build(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, double eta, double *Sigma) {
+  int rc = check_plan(p);
+  if (rc) return rc;
+  if (!Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "mp2_build: Sigma must be non-NULL");
+  if ((rc = do_begin(p, B, eps, occ, eta))) return rc;
+  if ((rc = mp2_direct_chunks(p))) { p->begun = false; return rc; }
+  if ((rc = mp2_sox_chunks(p))) { p->begun = false; return rc; }
   return do_finish(p, Sigma);
 }
 
@@ -569,7 +628,7 @@ int qsgw_sigma_destroy(qsgw_sigma_plan *p) {
     cudaFree(p->hOmega[b]); cudaFree(p->hZ[b]);
   }
   cudaFree(p->hB); cudaFree(p->hEps); cudaFree(p->hOcc); cudaFree(p->hSigma);
-  cudaFree(p->Bp); cudaFree(p->BovT); cudaFree(p->V); cudaFree(p->W); cudaFree(p->Tpart); cudaFree(p->pairs); cudaFree(p->mp2_omega);
+  cudaFree(p->Bp); cudaFree(p->BovT); cudaFree(p->V); cudaFree(p->W); cudaFree(p->Tpart); cudaFree(p->pairs); cudaFree(p->mp2_omega); cudaFree(p->mp2_y);
   cudaGetLastError();
   delete p;
   return QSGW_SIGMA_OK;

@@ -64,6 +64,18 @@ __global__ void mp2_chunk_kernel(const double *__restrict__ B, const double *__r
   else Omega[j] = eps[a] - eps[i];
 }
 
+// Exchange (SOX) term of qsMP2 at fixed occupied i: the virtual states a = a0 + j take the place of the poles.
+// blockIdx.y < n_aux: V[P][j] = B[P][i][a] (0 for a < n_occ: a0 may start one state early to stay 16-byte aligned);
+// blockIdx.y == n_aux: Omega[j] = eps_a - eps_i.
+__global__ void mp2_sox_chunk_kernel(const double *__restrict__ B, const double *__restrict__ eps, int n_mo, int n_occ, int n_aux,
+                                     int i, int a0, int sc, double *__restrict__ V, int64_t ldv, double *__restrict__ Omega) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= sc) return;
+  const int a = a0 + j, P = blockIdx.y;
+  if (P < n_aux) V[(int64_t)P * ldv + j] = (a >= n_occ) ? B[((int64_t)P * n_mo + i) * n_mo + a] : 0.0;
+  else Omega[j] = eps[a] - eps[i];
+}
+
 // ---------------------------------------------------------------- stage 3
 // D(m,s,omega) = occ_m * x1/(x1^2+eta^2) + (1-occ_m) * x2/(x2^2+eta^2),  x1 = (omega-eps_m)+Omega_s,
 // x2 = (omega-eps_m)-Omega_s: real part of the two terms of Eq. (17).  d = omega - eps_m.
@@ -167,7 +179,8 @@ __device__ __forceinline__ void mma_ktile_sigma_ragged(double (&acc)[4][8][2], c
 
 // One CTA: output tile (tp, tq) of T, 64 x 256, for the internal states m in [z*m_per_split, ...) and all
 // s_c poles of the chunk.  k-tiles of 16 poles at fixed m, so eps_m / occ_m are CTA-uniform per k-tile.
-//   W     [N*N][ldw]  chunk of residues, row m*N + p, column s (stage-2 output; both mirrors present)
+//   WA    [N*N][ldA]  left operand (scaled by D): row m*N + p, column s.  qsGW: the w chunk of stage 2 (both mirrors present)
+//   WB    [N*N][ldB]  right operand, same indexing.  qsGW: the same array; qsMP2 exchange term: (pi|an) left, -(mp|ia) right
 //   Omega [s_c]       excitation energies of the chunk
 //   Tpart [nsplit][N][N]  split-K partial tiles; slot z is owned by the CTAs with blockIdx.y == z and is
 //                     read-modify-written once per launch -> accumulation order is fixed, results reproducible.
@@ -175,9 +188,9 @@ __device__ __forceinline__ void mma_ktile_sigma_ragged(double (&acc)[4][8][2], c
 // ahead; each producer thread then multiplies the chunks of the p rows it copied itself by D(m, s, eps_p) in
 // place: the scaled operand A = w.D exists only in shared memory.  The 8 consumer warps run LDS + DMMA only.
 __global__ void __launch_bounds__(kThreads, 1)
-sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double *__restrict__ eps,
-                        const double *__restrict__ occ, const double *__restrict__ Omega, int n_mo, int s_c,
-                        double eta2, int m_per_split, int ntq, double *__restrict__ Tpart) {
+sigma_accumulate_kernel(const double *__restrict__ WA, int64_t ldA, const double *__restrict__ WB, int64_t ldB,
+                        const double *__restrict__ eps, const double *__restrict__ occ, const double *__restrict__ Omega,
+                        int n_mo, int s_c, double eta2, int m_per_split, int ntq, double *__restrict__ Tpart) {
   extern __shared__ __align__(16) double smem[];
   // stage st: p rows at smem + st*kSigmaStageDoubles (already scaled by D when released), q rows kTP*kBK further
   uint64_t *full = reinterpret_cast<uint64_t *>(smem + kSigmaStages * kSigmaStageDoubles);
@@ -213,7 +226,7 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
     double eps_p[kTP / 16];
 #pragma unroll
     for (int j = 0; j < kTP / 16; ++j) eps_p[j] = (j < nrowA) ? __ldg(eps + p0 + rA0 + 4 * j) : 0.0;
-    const int64_t row_step = 4 * ldw;
+    const int64_t stepA = 4 * ldA, stepB = 4 * ldB;
     constexpr int kAhead = 2;                     // k-tiles whose cp.async are in flight ahead of the scaling
 
     // loader: raw w rows of both operands, global -> shared (cp.async); every thread later scales exactly the
@@ -225,19 +238,19 @@ sigma_accumulate_kernel(const double *__restrict__ W, int64_t ldw, const double 
         mbar_wait(empty + ld_st, ld_ph);
         const int s = ld_ks * kBK + c2;
         const int ncol = min(2, max(0, s_c - s));
-        const double *srcA = W + ((int64_t)ld_m * n_mo + p0 + rA0) * ldw + s;
-        const double *srcB = W + ((int64_t)ld_m * n_mo + q0 + rB0) * ldw + s;
+        const double *srcA = WA + ((int64_t)ld_m * n_mo + p0 + rA0) * ldA + s;
+        const double *srcB = WB + ((int64_t)ld_m * n_mo + q0 + rB0) * ldB + s;
         double *dstA = smem + ld_st * kSigmaStageDoubles + rA0 * kBK + csw;
         double *dstB = smem + ld_st * kSigmaStageDoubles + (kTP + rB0) * kBK + csw;
 #pragma unroll
         for (int j = 0; j < kTP / 16; ++j) {
           const int nb = (j < nrowA) ? ncol * 8 : 0;
-          cp_async_16(dstA + 4 * j * kBK, nb ? srcA + j * row_step : W, nb);
+          cp_async_16(dstA + 4 * j * kBK, nb ? srcA + j * stepA : WA, nb);
         }
 #pragma unroll
         for (int j = 0; j < kTQ / 16; ++j) {
           const int nb = (j < nrowB) ? ncol * 8 : 0;
-          cp_async_16(dstB + 4 * j * kBK, nb ? srcB + j * row_step : W, nb);
+          cp_async_16(dstB + 4 * j * kBK, nb ? srcB + j * stepB : WB, nb);
         }
         if (++ld_ks == KTS) { ld_ks = 0; ++ld_m; }
         if (++ld_st == kSigmaStages) { ld_st = 0; ld_ph ^= 1; }

@@ -39,3 +39,31 @@ def test_parity(n_mo, n_occ, n_aux, s_block):
                                 torch.eye(cfg.n_ov, dtype=torch.float64, device="cuda"), cfg.eta)
     assert float((S_gw - S).abs().max()) <= 1e-11 * float(S.abs().max())
     pkg.qsgw_sigma_destroy(plan)
+
+
+@pytest.mark.parametrize("n_mo,n_occ,n_aux,s_block", [
+    (24, 5, 80, 0),        # odd n_occ: the exchange loop starts one (zero-weight) state early to stay aligned
+    (37, 7, 53, 8),        # odd N (padded exchange-integral rows, scalar GEMM loads), virtual range cut into several chunks
+    (120, 20, 400, 512),   # small config shapes
+    (70, 64, 33, 0),       # few virtual states
+    (2, 1, 1, 0),
+])
+def test_full_qsmp2_parity(n_mo, n_occ, n_aux, s_block):
+    """direct + second-order exchange (qsgw_mp2_build) against oracle.mp2; the exchange part alone as the difference of
+    the two entry points against the oracle's sox_only mode."""
+    pkg = _pkg()
+    cfg = qi.custom_config(n_mo, n_occ, n_aux, s_block=s_block, seed=700 + n_mo)
+    B, eps, occ = qi.make_B(cfg), qi.make_eps(cfg), qi.make_occ(cfg)
+    plan = pkg.qsgw_sigma_create(n_mo, n_occ, n_aux, cfg.n_ov, s_block)
+    Bd, ed, od = B.cuda(), eps.cuda(), occ.cuda()
+    S = pkg.qsgw_mp2_build(plan, Bd, ed, od, cfg.eta)
+    Sd = pkg.qsgw_mp2_direct_build(plan, Bd, ed, od, cfg.eta)
+    torch.cuda.synchronize()
+    ref = oracle.mp2(B.numpy(), eps.numpy(), occ.numpy(), cfg.eta, n_occ)
+    ref_sox = oracle.mp2(B.numpy(), eps.numpy(), occ.numpy(), cfg.eta, n_occ, sox_only=True)
+    scale = np.abs(ref).max()
+    assert np.max(np.abs(S.cpu().numpy() - ref)) <= 1e-9 * scale
+    assert np.max(np.abs((S - Sd).cpu().numpy() - ref_sox)) <= 1e-9 * max(np.abs(ref_sox).max(), 1e-300) + 1e-12 * scale
+    assert torch.equal(S, S.T)
+    assert torch.equal(S, pkg.qsgw_mp2_build(plan, Bd, ed, od, cfg.eta))       # reproducible
+    pkg.qsgw_sigma_destroy(plan)
