@@ -488,6 +488,71 @@ def run_gpu_aomo(args):
     return 0
 
 
+def run_gpu_mp2(args):
+    """--path mp2: row 8(f).3, one qsgw_mp2_build (direct + second-order exchange sums of Eq. (20) in Eq. (21)) on the
+    workload's B, eps, occ.  Flop model (2 per FMA): direct = F2sym + F3 with n_s = o*v; exchange, per occupied i:
+    2 N^2 v naux (exchange integrals) + 2 [N(N+1)/2] v naux (stage 2) + 2 N^3 v (stage 3)."""
+    import torch
+    import qsgw_inputs as qi
+    import paper_2210_17093_b200 as pkg
+
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("--path mp2 is a single-GPU measurement")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    cfg = qi.CONFIGS[args.workload]
+    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak, peak_src, _ = fp64_peak_tflops(nsm)
+    B = qi.make_B(cfg, dev)
+    eps, occ = qi.make_eps(cfg).to(dev), qi.make_occ(cfg).to(dev)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_ov, cfg.s_block)
+    pkg.qsgw_sigma_set_profiling(plan, True)
+    S = torch.empty((cfg.n_mo, cfg.n_mo), dtype=torch.float64, device=dev)
+    for _ in range(args.warmup):
+        pkg.qsgw_mp2_build(plan, B, eps, occ, cfg.eta, S)
+    torch.cuda.synchronize()
+    pkg.qsgw_sigma_get_stats(plan, reset=True)
+    evs = []
+    with ClockSampler(0) as clocks:
+        for _ in range(args.steps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); pkg.qsgw_mp2_build(plan, B, eps, occ, cfg.eta, S); e1.record()
+            evs.append((e0, e1))
+        torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps
+    stats = pkg.qsgw_sigma_get_stats(plan, reset=True)
+    assert torch.isfinite(S).all()
+    N, o, v, naux = float(cfg.n_mo), float(cfg.n_occ), float(cfg.n_virt), float(cfg.n_aux)
+    npair = N * (N + 1) / 2
+    f_direct = 2 * npair * naux * o * v + 2 * N ** 3 * o * v
+    f_sox = o * (2 * N * N * v * naux + 2 * npair * v * naux + 2 * N ** 3 * v)
+    val = (f_direct + f_sox) / (ms * 1e-3) / 1e12
+    out = {"metric": "qsmp2_sigma_c_build_fp64_tflops", "value": val, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic", "path": "mp2 (SURVEY.md 8(f).3)",
+           "config": _config_dict(cfg, args, extra={"flops_direct": f_direct, "flops_exchange": f_sox}),
+           "stage_ms_per_build": {"pack": stats["ms_pack"] / args.steps, "gemms": stats["ms_stage2"] / args.steps,
+                                  "stage3": stats["ms_stage3"] / args.steps, "epilogue": stats["ms_epilogue"] / args.steps},
+           "roofline": {"bound": "tensor", "kernel": "whole build (GEMMs + sigma_accumulate_kernel)", "achieved": val, "peak": peak,
+                        "unit": UNIT, "frac": val / peak, "launches": stats["kernel_launches"], "avg_launch_ms": None, "traffic": None,
+                        "peak_source": f"FP64 pipe rate at max SM clock ({peak_src})"},
+           "gpu_launches": stats["kernel_launches"], "clocks": clocks.summary(),
+           "e2e": {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                   "how": "B, eps, occ stay on the device between the AO->MO transform and the build"}}
+    if not args.no_cpu_baseline and cfg.n_mo <= 120:
+        import oracle
+        t0 = time.perf_counter()
+        oracle.mp2(B.cpu().numpy(), eps.cpu().numpy(), occ.cpu().numpy(), cfg.eta, cfg.n_occ)
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": (f_direct + f_sox) / dt / 1e12, "unit": UNIT + " (GPU flop model / oracle time)",
+                               "cores": oracle.num_threads(), "kind": "oracle", "sample": f"whole '{cfg.name}' build ({dt:.1f} s)"}
+    print(json.dumps(out), flush=True)
+    pkg.qsgw_sigma_destroy(plan)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -501,7 +566,7 @@ def main():
     ap.add_argument("--e2e-warmup", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-poles", type=int, default=0, help="poles in the oracle's timed sample (0 = auto, ~20 s)")
-    ap.add_argument("--path", default="sigma", choices=["sigma", "diag", "aomo"],
+    ap.add_argument("--path", default="sigma", choices=["sigma", "diag", "aomo", "mp2"],
                     help="sigma: the qsGW Sigma^c build (the bench contract); diag: the G0W0 diagonal on a frequency grid")
     ap.add_argument("--n-omega", type=int, default=64, help="grid points of --path diag")
     args = ap.parse_args()
@@ -513,6 +578,8 @@ def main():
         return run_gpu_diag(args)
     if args.path == "aomo":
         return run_gpu_aomo(args)
+    if args.path == "mp2":
+        return run_gpu_mp2(args)
     return run_gpu(args)
 
 
