@@ -286,7 +286,7 @@ def run_gpu(args):
             "stage_tflops": {"stage1": fl["F1"] * args.steps / max(stats["ms_stage1"], 1e-9) / 1e9,
                              "stage2": fl["F2sym"] * args.steps / max(stats["ms_stage2"], 1e-9) / 1e9,
                              "stage3": fl["F3"] * args.steps / max(stats["ms_stage3"], 1e-9) / 1e9},
-            "roofline": {"bound": "tensor", "kernel": "gemm_tn_dmma_kernel<2,EpiPairScatter> (stage 2, w producer)",
+            "roofline": {"bound": "tensor", "kernel": "gemm_tn_dmma_kernel<2,2,EpiPairScatter> (stage 2, w producer)",
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "launches": stats["launches_stage2"], "avg_launch_ms": s2_ms,
                          "traffic": NCU_STAGE2_DRAM_BYTES_PER_LAUNCH.get(cfg.name), "traffic_unit": "bytes per launch (dram read + write, ncu --set full, profiles/r01_full_large.md)",

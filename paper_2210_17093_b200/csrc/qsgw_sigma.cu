@@ -370,7 +370,7 @@ int ensure_host_staging(qsgw_sigma_plan *p) {
 
 extern "C" {
 
-int qsgw_sigma_version(void) { return 100; }
+int qsgw_sigma_version(void) { return 10100; }
 
 int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, int64_t n_pole_max, int s_block,
                       void *cuda_stream) {
