@@ -33,7 +33,7 @@ UNIT = "TFLOP/s"
 # FP64 pipe of sm_100a: DMMA.8x8x4 and DFMA both retire 64 FMA/clk/SM (measured: profiles/r01_fp64_peaks.md)
 FP64_FMA_PER_CLK_PER_SM = 64
 # dram__bytes_read.sum + dram__bytes_write.sum of one stage-2 launch over a full s-block (profiles/r01_full_large.md)
-NCU_STAGE2_DRAM_BYTES_PER_LAUNCH = {"large": 37.488597e9 + 11.782985e9}
+NCU_STAGE2_DRAM_BYTES_PER_LAUNCH = {"large": 38.731918e9 + 11.789630e9}
 
 
 def _peaks():
