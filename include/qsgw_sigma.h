@@ -195,6 +195,12 @@ const char *qsgw_sigma_last_error(const qsgw_sigma_plan *plan);
 /* Device bytes the plan allocated (workspace + host-path staging so far). */
 size_t qsgw_sigma_workspace_bytes(const qsgw_sigma_plan *plan);
 
+/* Bounds the number of poles one stage-1 launch handles (default: as many as fit in 4 GiB of V, at most n_pole_max).  A
+ * build / add_poles call with more poles runs stage 1 range by range; the result does not depend on it beyond rounding
+ * order (V is the same, the chunks of stages 2-3 are cut at other places only if n is not a multiple of s_block).
+ * n is rounded up to a multiple of the plan's s_block and clamped to the allocated capacity.  INVALID_ARG if n < 1. */
+int qsgw_sigma_limit_pole_batch(qsgw_sigma_plan *plan, int64_t n);
+
 /* Profiling on (1) / off (0): when on, every kernel launch is bracketed by CUDA events on the plan's
  * stream and qsgw_sigma_get_stats sums them per stage.  Off by default. */
 int qsgw_sigma_set_profiling(qsgw_sigma_plan *plan, int on);

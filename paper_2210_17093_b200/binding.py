@@ -23,7 +23,7 @@ QSGW_SIGMA_ERR_CUDA = -3
 EXPORTS = (
     "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
     "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_mp2_direct_build", "qsgw_mp2_build", "qsgw_ri_ao_to_mo", "qsgw_ri_ao_to_mo_work_doubles", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
-    "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_copy_workspace", "qsgw_sigma_version", "qsgw_sigma_fp64_probe",
+    "qsgw_sigma_limit_pole_batch", "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_copy_workspace", "qsgw_sigma_version", "qsgw_sigma_fp64_probe",
 )
 
 
@@ -89,6 +89,8 @@ def load_library() -> ctypes.CDLL:
         lib.qsgw_sigma_last_error.argtypes = [vp]
         lib.qsgw_sigma_workspace_bytes.restype = ctypes.c_size_t
         lib.qsgw_sigma_workspace_bytes.argtypes = [vp]
+        lib.qsgw_sigma_limit_pole_batch.restype = ci
+        lib.qsgw_sigma_limit_pole_batch.argtypes = [vp, i64]
         lib.qsgw_sigma_set_profiling.restype = ci
         lib.qsgw_sigma_set_profiling.argtypes = [vp, ci]
         lib.qsgw_sigma_get_stats.restype = ci
@@ -302,6 +304,10 @@ def qsgw_sigma_last_error(plan: Optional[Plan]) -> str:
 
 def qsgw_sigma_workspace_bytes(plan: Plan) -> int:
     return int(load_library().qsgw_sigma_workspace_bytes(plan.handle))
+
+
+def qsgw_sigma_limit_pole_batch(plan: Plan, n: int) -> None:
+    _check(load_library().qsgw_sigma_limit_pole_batch(plan.handle, int(n)), plan.handle)
 
 
 def qsgw_sigma_set_profiling(plan: Plan, on: bool) -> None:

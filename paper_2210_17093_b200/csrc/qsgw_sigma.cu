@@ -36,7 +36,8 @@ struct qsgw_sigma_plan {
   int n_mo = 0, n_occ = 0, n_virt = 0, n_aux = 0;
   int64_t n_ov = 0, n_pole_max = 0;
   int s_chunk = 0;
-  int64_t v_cols = 0;   // poles per stage-1 launch (V holds this many columns)
+  int64_t v_cols = 0;   // poles per stage-1 launch (<= v_cols_alloc)
+  int64_t v_cols_alloc = 0;   // columns of V that are allocated
   cudaStream_t stream = nullptr;
   int device = 0, num_sms = 0;
 
@@ -416,6 +417,7 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
     p->v_cols = std::min<int64_t>(round_up(n_pole_max, 2), cap);
   }
   p->ldv = round_up(p->v_cols, 2);
+  p->v_cols_alloc = p->v_cols;
   p->ldw = round_up(p->s_chunk, 2);
   // split-K of stage 3 over the internal state m: enough CTAs for ~40 waves of the SMs (ragged edge tiles run 2-3x shorter than full ones: the tail of a launch is one CTA long), at most N splits
   const int nt2 = ((n_mo + kTP - 1) / kTP) * ((n_mo + kTQ - 1) / kTQ);
@@ -637,6 +639,13 @@ int qsgw_sigma_destroy(qsgw_sigma_plan *p) {
 const char *qsgw_sigma_last_error(const qsgw_sigma_plan *p) { return p ? p->err.c_str() : g_create_error.c_str(); }
 
 size_t qsgw_sigma_workspace_bytes(const qsgw_sigma_plan *p) { return p ? p->bytes : 0; }
+
+int qsgw_sigma_limit_pole_batch(qsgw_sigma_plan *p, int64_t n) {
+  if (!p) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "plan is NULL");
+  if (n < 1) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "limit_pole_batch: n < 1");
+  p->v_cols = std::min<int64_t>(p->v_cols_alloc, round_up(n, p->s_chunk));
+  return QSGW_SIGMA_OK;
+}
 
 int qsgw_sigma_set_profiling(qsgw_sigma_plan *p, int on) {
   if (!p) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "plan is NULL");

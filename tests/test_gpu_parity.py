@@ -151,6 +151,23 @@ def test_additive_over_pole_ranges_and_chunkings():
     pkg.qsgw_sigma_destroy(plan)
 
 
+def test_stage1_in_several_pole_batches():
+    """more poles in one call than one stage-1 launch takes (V capacity): the v-range loop of add_poles"""
+    pkg = _pkg()
+    cfg = qi.custom_config(50, 8, 31, n_pole=330, s_block=64, seed=44)
+    inp = qi.make_inputs(cfg)
+    dev = _to_dev(inp)
+    ref = _ref_sigma(cfg, inp)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, cfg.s_block)
+    S_one = pkg.qsgw_sigma_build(plan, *dev, cfg.eta).clone()
+    for batch in (1, 64, 100, 256):                       # rounded up to 64, 64, 128, 256 poles per stage-1 launch
+        pkg.qsgw_sigma_limit_pole_batch(plan, batch)
+        S = pkg.qsgw_sigma_build(plan, *dev, cfg.eta)
+        _assert_parity(S, ref)
+        assert float((S - S_one).abs().max()) <= 1e-12 * float(S_one.abs().max())
+    pkg.qsgw_sigma_destroy(plan)
+
+
 def test_host_buffer_entry_point_matches_device_entry_point():
     pkg = _pkg()
     cfg = qi.custom_config(64, 10, 48, n_pole=540, s_block=128, seed=21)
