@@ -164,3 +164,47 @@ def test_xl_config_streamed_build_separable_closed_form():
     got = S.cpu().numpy()[np.ix_(states, states)]
     _assert_parity(got, ref, "xl, separable closed form")
     pkg.qsgw_sigma_destroy(plan)
+
+
+def test_large_config_g0w0_diagonal_pole_subrange_vs_oracle_on_sampled_states():
+    """Row 8(f).1 at the full N, naux, (ia) of `large`: 1024 poles straddling the s-block edge, 8 grid points, sampled
+    states against oracle.sigma_diag."""
+    pkg = _pkg()
+    cfg = qi.CONFIGS["large"]
+    dev = torch.device("cuda", 0)
+    s0, s1 = 4096 - 500, 4096 + 524
+    B = qi.make_B(cfg, dev)
+    eps, occ, Om = qi.make_eps(cfg), qi.make_occ(cfg), qi.make_omega(cfg)
+    eps_d, occ_d, Om_d = eps.to(dev), occ.to(dev), Om.to(dev)
+    Zr = qi.make_Z(cfg, s0, s1, device=dev)
+    grid = np.array([-2.0, float(eps[cfg.n_occ - 1]), float(eps[cfg.n_occ]), 0.0, 0.731, float(eps[0] - Om[s0 + 3]), 3.3, 6.5])
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, cfg.s_block)
+    re, im = pkg.qsgw_sigma_diag_build(plan, B, eps_d, occ_d, Om_d[s0:s1], Zr, cfg.eta, torch.from_numpy(grid).to(dev))
+    torch.cuda.synchronize()
+    states = _sample_states(cfg, n_random=2, seed=3)
+    ref_re, ref_im = oracle.sigma_diag(B.cpu().numpy(), eps.numpy(), occ.numpy(), Om.numpy()[s0:s1], Zr.cpu().numpy(),
+                                       cfg.eta, cfg.n_occ, grid, states=states)
+    _assert_parity(re.cpu().numpy()[states], ref_re, "large, G0W0 diagonal Re")
+    _assert_parity(im.cpu().numpy()[states], ref_im, "large, G0W0 diagonal Im")
+    pkg.qsgw_sigma_destroy(plan)
+
+
+def test_large_config_ao_to_mo_sampled_auxiliary_functions():
+    """Row 8(f).2 at `large` (n_ao = N = 600, naux = 2400), as bench.py --path aomo runs it; the oracle transforms
+    a sample of the auxiliary functions (each P is independent)."""
+    pkg = _pkg()
+    cfg = qi.CONFIGS["large"]
+    dev = torch.device("cuda", 0)
+    B_ao = qi.make_B(cfg, dev)
+    g = torch.Generator(device=dev); g.manual_seed(11)
+    C, _ = torch.linalg.qr(torch.randn((cfg.n_mo, cfg.n_mo), generator=g, dtype=torch.float64, device=dev))
+    C = C.contiguous()
+    B_mo = pkg.qsgw_ri_ao_to_mo(B_ao, C)
+    torch.cuda.synchronize()
+    sample = [0, 1, 127, 128, 1199, 2398, 2399]
+    ref = oracle.ao_to_mo(B_ao[sample].cpu().numpy(), C.cpu().numpy())
+    _assert_parity(B_mo[sample].cpu().numpy(), ref, "large, AO->MO")
+    # an orthogonal C preserves the trace of every B[P]: a property checked on ALL 2400 auxiliary functions
+    tr_ao = torch.diagonal(B_ao, dim1=1, dim2=2).sum(-1)
+    tr_mo = torch.diagonal(B_mo, dim1=1, dim2=2).sum(-1)
+    assert float((tr_ao - tr_mo).abs().max()) <= 1e-10 * float(B_ao.abs().max()) * cfg.n_mo
