@@ -66,3 +66,15 @@ def test_product_does_not_import_or_link_the_oracle():
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2210_17093_b200" not in text and "from paper_2210_17093_b200" not in text
             assert "csrc" not in text or f.endswith(".c")   # the C file only names csrc/ in its header comment
+
+
+def test_stats_struct_layout_matches_the_header():
+    """The ctypes mirror of qsgw_sigma_stats must list the header's fields in the header's order with the header's types."""
+    from paper_2210_17093_b200 import binding
+    text = open(os.path.join(ROOT, "include", "qsgw_sigma.h")).read()
+    body = re.search(r"typedef struct qsgw_sigma_stats \{(.*?)\} qsgw_sigma_stats;", text, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    declared = [(t, n) for t, n in re.findall(r"\b(double|int64_t)\s+(\w+)\s*;", body)]
+    mirror = [("double" if c is ctypes.c_double else "int64_t", n) for n, c in binding.qsgw_sigma_stats._fields_]
+    assert declared == mirror
+    assert ctypes.sizeof(binding.qsgw_sigma_stats) == 8 * len(declared)
