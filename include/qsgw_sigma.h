@@ -24,13 +24,23 @@
  *     "host" pointers are ordinary host memory (pinned memory makes the copies faster, it is not required).
  *   - The caller owns every array it passes.  The plan owns its workspace (packed copies of B,
  *     V, the w chunk, split-K partial tiles), allocated in qsgw_sigma_create, freed in
- *     qsgw_sigma_destroy.  No build call allocates device memory.
+ *     qsgw_sigma_destroy.  qsgw_sigma_build / _begin / _add_poles / _finish / _diag_build never
+ *     allocate.  Three entry points allocate extra plan-owned device buffers on their FIRST call
+ *     (kept until destroy; ALLOC if they do not fit): qsgw_sigma_build_host (device copies of B,
+ *     eps, occ, Sigma and two Omega/Z ranges), qsgw_mp2_direct_build (one s_block of doubles) and
+ *     qsgw_mp2_build (that plus n_mo^3 doubles).
+ *   - Every entry point that takes a plan makes the plan's device current while it runs and
+ *     restores the caller's current device before it returns.
  *   - Device entry points are asynchronous on the plan's stream: inputs must stay alive and
  *     unmodified, and Sigma must not be read, until the stream has been synchronised.
  *   - Return value: QSGW_SIGMA_OK (0) or a negative qsgw_sigma_status.  No exception or abort
  *     crosses the ABI.  qsgw_sigma_last_error(plan) gives a message for the last failure.
- *   - Preconditions that would need a look at device data are NOT checked:
- *     B[P][p][q] == B[P][q][p] (real orbitals), occ[m] in [0,1], Omega[s] > 0.
+ *   - Preconditions that need a look at device data are checked only in DEBUG MODE
+ *     (qsgw_sigma_set_debug(plan, 1), or the environment variable QSGW_SIGMA_DEBUG=1 at create):
+ *     B[P][p][q] == B[P][q][p] to 1e-10 max|B| and finite (real orbitals), occ[m] in
+ *     [0,1], Omega[s] finite and > 0.  In debug mode begin / add_poles (and every build call made
+ *     of them) run small check kernels, SYNCHRONISE the stream and return INVALID_ARG with a
+ *     message if a precondition fails.  Outside debug mode they are not checked.
  */
 #ifndef QSGW_SIGMA_H
 #define QSGW_SIGMA_H
@@ -207,20 +217,19 @@ int qsgw_sigma_set_profiling(qsgw_sigma_plan *plan, int on);
 /* Synchronises the stream, fills *stats with the totals since the last reset; reset != 0 clears them. */
 int qsgw_sigma_get_stats(qsgw_sigma_plan *plan, qsgw_sigma_stats *stats, int reset);
 
-/* Test/debug helper: copy the leading rows x cols block of a workspace array into a dense device buffer
+/* Debug mode on (1) / off (0): device-side precondition checks in begin / add_poles (see "Preconditions" above).
+ * Off by default unless QSGW_SIGMA_DEBUG=1 was set when the plan was created. */
+int qsgw_sigma_set_debug(qsgw_sigma_plan *plan, int on);
+
+#ifdef QSGW_SIGMA_TEST_HOOKS
+/* Test hook, compiled only into the test build of the library (-DQSGW_SIGMA_TEST_HOOKS; libqsgw_sigma_testhooks.so),
+ * not into libqsgw_sigma.so: copy the leading rows x cols block of a workspace array into a dense device buffer
  * dst[rows][cols], asynchronously on the plan's stream.  which: 0 = V of the last chunk [n_aux][s],
  * 1 = w chunk of the last chunk [n_mo*n_mo][s] (row m*n_mo+p), 2 = packed symmetric B [n_aux][n_mo(n_mo+1)/2],
  * 3 = transposed ov block [n_occ*n_virt][n_aux], 4 = split-K partial tiles [nsplit][n_mo*n_mo] (rows = nsplit).
  * INVALID_ARG if the block exceeds the array. */
 int qsgw_sigma_copy_workspace(qsgw_sigma_plan *plan, int which, double *dst, int64_t rows, int64_t cols);
-
-/* Measurement helper (no plan needed): times a register-resident FP64 loop on every SM of the current device and
- * returns the achieved rate in *tflops (and the kernel time in *ms if non-NULL).  This is how the FP64 roofline
- * denominator (SMs x 64 FMA/clk x 2 x SM clock) is checked on the box, MEASURED_PEAKS.json having no FP64 entry.
- *   mode 0: DMMA.8x8x4 only   1: DFMA only   2: 32 DMMA + `mix` DFMA per iteration (mix a multiple of 8)
- *   mode 3: DMMA fed by LDS.64 fragment loads (the GEMM inner loop without global traffic)
- * iters >= 1 loop iterations per warp; ctas_per_sm >= 1 CTAs of 256 threads per SM.  Synchronises the stream. */
-int qsgw_sigma_fp64_probe(int mode, int iters, int mix, int ctas_per_sm, void *cuda_stream, double *tflops, double *ms);
+#endif
 
 /* Library version (major*10000 + minor*100 + patch). */
 int qsgw_sigma_version(void);

@@ -41,8 +41,9 @@
  *
  * Further rows at the end of this file: qsgw_oracle_mp2_direct and qsgw_oracle_mp2 (Eqs. (20)-(21), PAPER.md:174-186;
  * pins in tests/test_oracle_mp2_pins.py: the hand-solved two-state rationals, a literal complex spin-orbital brute force
- * of both sums incl. unsymmetric B, identity with the GW oracle at Z = 1, SOX = -direct/2 for rank-one B).  The RI AO->MO
- * transformation (oracle.ao_to_mo) lives in qsgw_oracle.py as a numpy matmul; pins in tests/test_oracle_aomo_pins.py.
+ * of both sums incl. unsymmetric B, identity with the GW oracle at Z = 1, SOX = -direct/2 for rank-one B);
+ * qsgw_oracle_mp2_states (the same sums for sampled output states, pinned by equality with qsgw_oracle_mp2); and
+ * qsgw_oracle_ao_to_mo, the RI AO->MO transformation as its defining double sum (pins in tests/test_oracle_aomo_pins.py).
  *
  * Floating point: products and the P-, ia- and m-sums are plain double; the running sum
  * over poles s of step 3 is kept in long double so that the oracle's own rounding is far
@@ -312,5 +313,119 @@ int qsgw_oracle_mp2(int N, int o, int naux, const double *B, const double *eps, 
   }
   for (size_t k = 0; k < NN; ++k) Sigma[k] = (double)acc[k];
   free(acc); free(L); free(R); free(E);
+  return 0;
+}
+
+/* ---- qsMP2 restricted to sampled output states (for parity checks at sizes where the full sum is unaffordable) ------
+ * The same sums as qsgw_oracle_mp2 -- Eq. (20) in Eq. (21), every integral read literally,
+ * (xy|zw) = sum_P B[P][x][y] B[P][z][w] -- for the outputs Sigma[r][c] = <S_r|Sigma|S_c> with S = states[0..n_states).
+ * All internal sums (i, a, p, P) run over their full ranges.  The only difference from qsgw_oracle_mp2 is data movement:
+ * the entries of B that the restricted outputs need are first COPIED (no arithmetic) into dense arrays with the
+ * auxiliary index P contiguous,
+ *   Brow[r][y][P] = B[P][S_r][y],   Bcol[y][r][P] = B[P][y][S_r],   Bi[y][P] = B[P][y][i] (per i),
+ *   bia[P] = B[P][i][a],  bai[P] = B[P][a][i] (per pair),
+ * so that the sums over P do not stride through all of B for every (i, a) pair.  Per pair (i, a):
+ *   L[r][p] = (S_r p|ia)  = sum_P Brow[r][p][P] bia[P]
+ *   R[p][r] = (p S_r|ai)  = sum_P Bcol[p][r][P] bai[P]
+ *   E[p][r] = (p i|a S_r) = sum_P Bi[p][P]      Bcol[a][r][P]
+ *   Sigma[r][c] += 1/2 sum_p ( L[r][p] (cd R[p][c] - E[p][c]) Dd(i,a,p,eps[S_c]) + L[c][p] (cd R[p][r] - E[p][r]) Dd(i,a,p,eps[S_r]) )
+ * with cd = 2 (0 if sox_only) and Dd as in qsgw_oracle_mp2_direct.  Pinned by equality with qsgw_oracle_mp2 on small
+ * inputs incl. unsymmetric B (tests/test_oracle_mp2_pins.py).  Sigma is n_states x n_states row-major.  Returns 0 / -1. */
+int qsgw_oracle_mp2_states(int N, int o, int naux, const double *B, const double *eps, const double *occ, double eta,
+                           int sox_only, int n_states, const int *states, double *Sigma) {
+  if (N < 2 || o < 1 || o >= N || naux < 1 || !(eta > 0.0) || n_states < 1 || !states) return -1;
+  for (int r = 0; r < n_states; ++r) if (states[r] < 0 || states[r] >= N) return -1;
+  const size_t NN = (size_t)N * N, nS = (size_t)n_states, nP = (size_t)naux;
+  long double *acc = (long double *)malloc(sizeof(long double) * nS * nS);
+  double *Brow = (double *)malloc(sizeof(double) * nS * N * nP);
+  double *Bcol = (double *)malloc(sizeof(double) * (size_t)N * nS * nP);
+  double *Bi = (double *)malloc(sizeof(double) * (size_t)N * nP);
+  double *bia = (double *)malloc(sizeof(double) * nP);
+  double *bai = (double *)malloc(sizeof(double) * nP);
+  double *L = (double *)malloc(sizeof(double) * nS * N);
+  double *R = (double *)malloc(sizeof(double) * (size_t)N * nS);
+  double *E = (double *)malloc(sizeof(double) * (size_t)N * nS);
+  if (!acc || !Brow || !Bcol || !Bi || !bia || !bai || !L || !R || !E) {
+    free(acc); free(Brow); free(Bcol); free(Bi); free(bia); free(bai); free(L); free(R); free(E);
+    return -1;
+  }
+  for (size_t k = 0; k < nS * nS; ++k) acc[k] = 0.0L;
+#pragma omp parallel for schedule(static)
+  for (int y = 0; y < N; ++y)                                        /* copies only */
+    for (int r = 0; r < n_states; ++r)
+      for (int P = 0; P < naux; ++P) {
+        Brow[((size_t)r * N + y) * nP + P] = B[(size_t)P * NN + (size_t)states[r] * N + y];
+        Bcol[((size_t)y * nS + r) * nP + P] = B[(size_t)P * NN + (size_t)y * N + states[r]];
+      }
+  const double cd = sox_only ? 0.0 : 2.0;
+  for (int i = 0; i < o; ++i) {
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < N; ++y)                                      /* copy */
+      for (int P = 0; P < naux; ++P) Bi[(size_t)y * nP + P] = B[(size_t)P * NN + (size_t)y * N + i];
+    for (int a = o; a < N; ++a) {
+      for (int P = 0; P < naux; ++P) {                               /* copies */
+        bia[P] = B[(size_t)P * NN + (size_t)i * N + a];
+        bai[P] = B[(size_t)P * NN + (size_t)a * N + i];
+      }
+#pragma omp parallel for schedule(static)
+      for (int p = 0; p < N; ++p) {
+        for (int r = 0; r < n_states; ++r) {
+          const double *brow = Brow + ((size_t)r * N + p) * nP, *bcol = Bcol + ((size_t)p * nS + r) * nP;
+          const double *bi = Bi + (size_t)p * nP, *bax = Bcol + ((size_t)a * nS + r) * nP;
+          double l = 0.0, rr = 0.0, e = 0.0;
+          for (int P = 0; P < naux; ++P) {
+            l += brow[P] * bia[P];
+            rr += bcol[P] * bai[P];
+            e += bi[P] * bax[P];
+          }
+          L[(size_t)r * N + p] = l; R[(size_t)p * nS + r] = rr; E[(size_t)p * nS + r] = e;
+        }
+      }
+#pragma omp parallel for schedule(static)
+      for (int r = 0; r < n_states; ++r) {
+        for (int c = 0; c < n_states; ++c) {
+          const int m = states[r], n = states[c];
+          double t = 0.0;
+          for (int p = 0; p < N; ++p) {
+            const double om[2] = {eps[n], eps[m]};
+            const double num[2] = {L[(size_t)r * N + p] * (cd * R[(size_t)p * nS + c] - E[(size_t)p * nS + c]),
+                                   L[(size_t)c * N + p] * (cd * R[(size_t)p * nS + r] - E[(size_t)p * nS + r])};
+            for (int k = 0; k < 2; ++k) {
+              const double x1 = om[k] + eps[a] - eps[i] - eps[p];
+              const double x2 = om[k] + eps[i] - eps[a] - eps[p];
+              t += num[k] * (occ[p] * (x1 / (x1 * x1 + eta * eta)) + (1.0 - occ[p]) * (x2 / (x2 * x2 + eta * eta)));
+            }
+          }
+          acc[(size_t)r * nS + c] += 0.5L * (long double)t;
+        }
+      }
+    }
+  }
+  for (size_t k = 0; k < nS * nS; ++k) Sigma[k] = (double)acc[k];
+  free(acc); free(Brow); free(Bcol); free(Bi); free(bia); free(bai); free(L); free(R); free(E);
+  return 0;
+}
+
+/* ---- row 8(f).2: RI AO->MO transformation of the three-index factors ------------------------------------------------
+ * The RI analogue of Eq. (16) (RI remark PAPER.md:120), the defining double sum written out for every
+ * auxiliary function P and every orbital pair (p, q):
+ *   B_mo[P][p][q] = sum_mu sum_nu C[mu][p] * C[nu][q] * B_ao[P][mu][nu]
+ * B_ao [naux][nao][nao] (not assumed symmetric), C [nao][nmo] (column p = orbital p), B_mo [naux][nmo][nmo], row-major.
+ * O(naux nmo^2 nao^2): callers sample the auxiliary index at large sizes (each P is independent).  Returns 0 / -1. */
+int qsgw_oracle_ao_to_mo(int naux, int nao, int nmo, const double *B_ao, const double *C, double *B_mo) {
+  if (naux < 1 || nao < 1 || nmo < 1) return -1;
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int P = 0; P < naux; ++P) {
+    for (int p = 0; p < nmo; ++p) {
+      double *row = B_mo + ((size_t)P * nmo + p) * nmo;              /* row[q] = B_mo[P][p][q], all q at once */
+      for (int q = 0; q < nmo; ++q) row[q] = 0.0;
+      for (int mu = 0; mu < nao; ++mu) {
+        for (int nu = 0; nu < nao; ++nu) {
+          const double cb = C[(size_t)mu * nmo + p] * B_ao[((size_t)P * nao + mu) * nao + nu];
+          for (int q = 0; q < nmo; ++q) row[q] += cb * C[(size_t)nu * nmo + q];
+        }
+      }
+    }
+  }
   return 0;
 }

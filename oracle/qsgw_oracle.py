@@ -57,6 +57,11 @@ def _load():
         lib.qsgw_oracle_mp2_direct.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, ctypes.c_double, dp]
         lib.qsgw_oracle_mp2.restype = ctypes.c_int
         lib.qsgw_oracle_mp2.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, ctypes.c_double, ctypes.c_int, dp]
+        lib.qsgw_oracle_mp2_states.restype = ctypes.c_int
+        lib.qsgw_oracle_mp2_states.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, ctypes.c_double, ctypes.c_int,
+                                               ctypes.c_int, ip, dp]
+        lib.qsgw_oracle_ao_to_mo.restype = ctypes.c_int
+        lib.qsgw_oracle_ao_to_mo.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp]
         _lib = lib
     return _lib
 
@@ -173,17 +178,23 @@ def sigma_diag(B, eps, occ, Omega, Z, eta: float, n_occ: int, omega, states=None
 
 def ao_to_mo(B_ao, C):
     """RI AO->MO transformation of the three-index factors: the RI analogue of Eq. (16)
-    (RI remark PAPER.md:120), B^P_pq = sum_mu sum_nu C[mu][p] C[nu][q] B^P_mu,nu, i.e. for every
-    auxiliary function P the matrix identity B_mo[P] = C^T B_ao[P] C, written with numpy's FP64 matmul as the step.
+    (RI remark PAPER.md:120), B^P_pq = sum_mu sum_nu C[mu][p] C[nu][q] B^P_mu,nu -- the defining double
+    sum in plain C loops (qsgw_oracle_ao_to_mo), O(naux n_mo^2 nao^2): pass a sample of the auxiliary functions at
+    large sizes (each P is independent).
 
     B_ao [naux, nao, nao], C [nao, n_mo] (AO coefficients of the MOs, column p = orbital p) -> [naux, n_mo, n_mo].
-    Pinned in tests/test_oracle_aomo_pins.py against the literal 4-deep double sum on tiny inputs and invariants.
+    Pinned in tests/test_oracle_aomo_pins.py (hand values, identity / permutation / selection, composition, trace).
     """
     B_ao = _f64(B_ao)
     C = _f64(C)
     if B_ao.ndim != 3 or B_ao.shape[1] != B_ao.shape[2] or C.ndim != 2 or C.shape[0] != B_ao.shape[1]:
         raise ValueError("need B_ao [naux, nao, nao] and C [nao, n_mo]")
-    return np.matmul(C.T[None, :, :], np.matmul(B_ao, C[None, :, :]))
+    naux, nao, n_mo = B_ao.shape[0], B_ao.shape[1], C.shape[1]
+    out = np.empty((naux, n_mo, n_mo))
+    rc = _load().qsgw_oracle_ao_to_mo(naux, nao, n_mo, _dp(B_ao), _dp(C), _dp(out))
+    if rc != 0:
+        raise RuntimeError(f"qsgw_oracle_ao_to_mo failed with {rc}")
+    return out
 
 
 def mp2_direct(B, eps, occ, eta: float, n_occ: int):
@@ -202,15 +213,29 @@ def mp2_direct(B, eps, occ, eta: float, n_occ: int):
     return out
 
 
-def mp2(B, eps, occ, eta: float, n_occ: int, sox_only: bool = False):
+def mp2(B, eps, occ, eta: float, n_occ: int, sox_only: bool = False, states=None):
     """qsMP2 correlation self-energy: both sums of Eq. (20) (direct and second-order exchange) in Eq. (21), closed
-    shell.  ``sox_only`` returns the exchange part alone.  Returns Sigma [N, N]."""
+    shell.  ``sox_only`` returns the exchange part alone.  Returns Sigma [N, N].
+
+    ``states`` (optional list of MO indices) restricts the OUTPUT to those rows/columns (qsgw_oracle_mp2_states: all
+    internal sums still run over their full ranges); returns [len(states), len(states)].
+    """
     B = _f64(B)
     naux, N, N2 = B.shape
     if N != N2:
         raise ValueError("B must be [naux, N, N]")
     eps = _f64(eps, (N,))
     occ = _f64(occ, (N,))
+    if states is not None:
+        keep = np.ascontiguousarray(states, dtype=np.int32)
+        if keep.ndim != 1 or len(keep) < 1 or keep.min() < 0 or keep.max() >= N:
+            raise ValueError("states out of range")
+        out = np.empty((len(keep), len(keep)))
+        rc = _load().qsgw_oracle_mp2_states(N, n_occ, naux, _dp(B), _dp(eps), _dp(occ), float(eta), 1 if sox_only else 0,
+                                            len(keep), keep.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), _dp(out))
+        if rc != 0:
+            raise RuntimeError(f"qsgw_oracle_mp2_states failed with {rc}")
+        return out
     out = np.empty((N, N))
     rc = _load().qsgw_oracle_mp2(N, n_occ, naux, _dp(B), _dp(eps), _dp(occ), float(eta), 1 if sox_only else 0, _dp(out))
     if rc != 0:

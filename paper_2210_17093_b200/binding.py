@@ -3,6 +3,11 @@
 Every step of the path runs in the CUDA kernels of libqsgw_sigma.so; PyTorch is used for
 device memory and streams.  There is no CPU fallback: if the shared library is missing or
 there is no CUDA device the calls raise.  Function names are the C names.
+
+Streams: a plan enqueues all its work on the stream it was created with.  Tensors handed to a
+plan must have been produced on that stream (or the caller must have made the stream wait for
+their producers), and must stay alive until the stream has passed the call -- the binding keeps
+no references.
 """
 from __future__ import annotations
 
@@ -23,7 +28,7 @@ QSGW_SIGMA_ERR_CUDA = -3
 EXPORTS = (
     "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
     "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_mp2_direct_build", "qsgw_mp2_build", "qsgw_ri_ao_to_mo", "qsgw_ri_ao_to_mo_work_doubles", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
-    "qsgw_sigma_limit_pole_batch", "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_copy_workspace", "qsgw_sigma_version", "qsgw_sigma_fp64_probe",
+    "qsgw_sigma_limit_pole_batch", "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_set_debug", "qsgw_sigma_version",
 )
 
 
@@ -95,10 +100,8 @@ def load_library() -> ctypes.CDLL:
         lib.qsgw_sigma_set_profiling.argtypes = [vp, ci]
         lib.qsgw_sigma_get_stats.restype = ci
         lib.qsgw_sigma_get_stats.argtypes = [vp, ctypes.POINTER(qsgw_sigma_stats), ci]
-        lib.qsgw_sigma_copy_workspace.restype = ci
-        lib.qsgw_sigma_copy_workspace.argtypes = [vp, ci, dp, i64, i64]
-        lib.qsgw_sigma_fp64_probe.restype = ci
-        lib.qsgw_sigma_fp64_probe.argtypes = [ci, ci, ci, ci, vp, ctypes.POINTER(cd), ctypes.POINTER(cd)]
+        lib.qsgw_sigma_set_debug.restype = ci
+        lib.qsgw_sigma_set_debug.argtypes = [vp, ci]
         lib.qsgw_sigma_version.restype = ci
         lib.qsgw_sigma_version.argtypes = []
         _lib = lib
@@ -130,9 +133,9 @@ def _host(t: torch.Tensor, name: str, shape=None) -> int:
 class Plan:
     """Handle returned by qsgw_sigma_create (holds the opaque qsgw_sigma_plan* and the sizes)."""
 
-    def __init__(self, handle, n_mo, n_occ, n_aux, n_pole_max, s_block, stream):
+    def __init__(self, handle, n_mo, n_occ, n_aux, n_pole_max, s_block, stream, device):
         self.handle, self.n_mo, self.n_occ, self.n_aux = handle, n_mo, n_occ, n_aux
-        self.n_pole_max, self.s_block, self.stream = n_pole_max, s_block, stream
+        self.n_pole_max, self.s_block, self.stream, self.device = n_pole_max, s_block, stream, device
         self.n_ov = n_occ * (n_mo - n_occ)
 
     def __del__(self):
@@ -144,14 +147,18 @@ class Plan:
 
 def qsgw_sigma_create(n_mo: int, n_occ: int, n_aux: int, n_pole_max: int, s_block: int = 0,
                       stream: Optional[torch.cuda.Stream] = None) -> Plan:
+    """The plan lives on the current CUDA device (the stream, if given, must belong to it)."""
     lib = load_library()
-    if stream is None and torch.cuda.is_available():
-        stream = torch.cuda.current_stream()
+    device = None
+    if torch.cuda.is_available():
+        if stream is None:
+            stream = torch.cuda.current_stream()
+        device = torch.device("cuda", torch.cuda.current_device())
     sptr = ctypes.c_void_p(stream.cuda_stream if stream is not None else 0)
     h = ctypes.c_void_p()
     rc = lib.qsgw_sigma_create(ctypes.byref(h), int(n_mo), int(n_occ), int(n_aux), int(n_pole_max), int(s_block), sptr)
     _check(rc, None)
-    return Plan(h, n_mo, n_occ, n_aux, n_pole_max, s_block, stream)
+    return Plan(h, n_mo, n_occ, n_aux, n_pole_max, s_block, stream, device)
 
 
 def _z_args(plan: Plan, Omega: torch.Tensor, Z: torch.Tensor, ptr):
@@ -195,7 +202,7 @@ def qsgw_sigma_add_poles(plan: Plan, Omega, Z) -> None:
 def qsgw_sigma_finish(plan: Plan, Sigma: Optional[torch.Tensor] = None) -> torch.Tensor:
     N = plan.n_mo
     if Sigma is None:
-        Sigma = torch.empty((N, N), dtype=torch.float64, device="cuda")
+        Sigma = torch.empty((N, N), dtype=torch.float64, device=plan.device)
     _check(load_library().qsgw_sigma_finish(plan.handle, _dev(Sigma, "Sigma", (N, N))), plan.handle)
     return Sigma
 
@@ -278,7 +285,9 @@ def qsgw_ri_ao_to_mo(B_ao: torch.Tensor, C: torch.Tensor, B_mo: Optional[torch.T
     if work.numel() < need or not work.is_contiguous():
         raise ValueError(f"work needs {need} contiguous doubles")
     if stream is None:
-        stream = torch.cuda.current_stream()
+        stream = torch.cuda.current_stream(B_ao.device)
+    for t in (B_ao, C, B_mo, work):       # the launch is asynchronous on `stream`: keep the allocator from reusing them early
+        t.record_stream(stream)
     rc = load_library().qsgw_ri_ao_to_mo(_dev(B_ao, "B_ao"), _dev(C, "C"), n_aux, n_ao, n_mo, _dev(work, "work"),
                                          _dev(B_mo, "B_mo", (n_aux, n_mo, n_mo)), ctypes.c_void_p(stream.cuda_stream))
     _check(rc, None)
@@ -320,26 +329,9 @@ def qsgw_sigma_get_stats(plan: Plan, reset: bool = False) -> dict:
     return st.as_dict()
 
 
-WORKSPACE_V, WORKSPACE_W, WORKSPACE_BP, WORKSPACE_BOVT, WORKSPACE_TPART = range(5)
-
-
-def qsgw_sigma_copy_workspace(plan: Plan, which: int, rows: int, cols: int) -> torch.Tensor:
-    """Test/debug helper: dense copy of the leading rows x cols block of a workspace array."""
-    out = torch.empty((rows, cols), dtype=torch.float64, device="cuda")
-    _check(load_library().qsgw_sigma_copy_workspace(plan.handle, int(which), out.data_ptr(), int(rows), int(cols)),
-           plan.handle)
-    return out
-
-
-def qsgw_sigma_fp64_probe(mode: int, iters: int = 20000, mix: int = 0, ctas_per_sm: int = 1) -> dict:
-    """Measured FP64 issue rate of the current device (mode 0 DMMA, 1 DFMA, 2 DMMA+DFMA mix, 3 LDS-fed DMMA)."""
-    tf, ms = ctypes.c_double(), ctypes.c_double()
-    sptr = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
-    rc = load_library().qsgw_sigma_fp64_probe(int(mode), int(iters), int(mix), int(ctas_per_sm), sptr,
-                                              ctypes.byref(tf), ctypes.byref(ms))
-    if rc != QSGW_SIGMA_OK:
-        raise QsgwSigmaError(rc, "fp64 probe failed")
-    return {"tflops": tf.value, "ms": ms.value}
+def qsgw_sigma_set_debug(plan: Plan, on: bool) -> None:
+    """Device-side precondition checks (B symmetric and finite, occ in [0,1], Omega > 0) in begin / add_poles."""
+    _check(load_library().qsgw_sigma_set_debug(plan.handle, 1 if on else 0), plan.handle)
 
 
 def qsgw_sigma_version() -> int:

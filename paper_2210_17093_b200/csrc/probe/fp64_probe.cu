@@ -1,4 +1,6 @@
 // fp64_probe.cu -- measures the FP64 issue rates the roofline of this library is quoted against.
+// MEASUREMENT TOOL, not part of the product: built into its own libqsgw_fp64_probe.so (paper_2210_17093_b200/build.py),
+// loaded only by bench.py; libqsgw_sigma.so neither contains nor calls it, and this file includes no product header.
 //
 // MEASURED_PEAKS.json carries no FP64 figure, so the denominator of the "fraction of FP64 tensor peak" is
 // derived (SMs x 64 FMA/clk x 2 x max SM clock) and CHECKED on the box by these register-resident loops:
@@ -10,10 +12,16 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "../../include/qsgw_sigma.h"
-#include "dmma_gemm.cuh"
+namespace qsgw_probe {
 
-namespace qsgw {
+constexpr int kBK = 16;          // k depth and padded row length of the shared tile in mode 3 (the GEMM kernels' layout)
+constexpr int kLdT = 128 + 4;
+
+__device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+      : "+d"(c[0]), "+d"(c[1])
+      : "d"(a), "d"(b));
+}
 
 template <int MODE>
 __global__ void __launch_bounds__(256) fp64_probe_kernel(int iters, int mix, double seed, double *sink) {
@@ -83,21 +91,22 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(int iters, int mix, dou
   if (s == 12345.678) sink[0] = s;   // never true for the seeds used; keeps the loops alive
 }
 
-}  // namespace qsgw
+}  // namespace qsgw_probe
 
-extern "C" int qsgw_sigma_fp64_probe(int mode, int iters, int mix, int ctas_per_sm, void *cuda_stream, double *tflops,
-                                     double *ms_out) {
-  using namespace qsgw;
-  if (mode < 0 || mode > 3 || iters < 1 || mix < 0 || (mix & 7) || ctas_per_sm < 1 || !tflops) return QSGW_SIGMA_ERR_INVALID_ARG;
+// Returns 0, or -1 bad argument, -2 allocation failure, -3 CUDA failure.  Synchronises the stream.
+extern "C" int qsgw_fp64_probe(int mode, int iters, int mix, int ctas_per_sm, void *cuda_stream, double *tflops,
+                               double *ms_out) {
+  using namespace qsgw_probe;
+  if (mode < 0 || mode > 3 || iters < 1 || mix < 0 || (mix & 7) || ctas_per_sm < 1 || !tflops) return -1;
   int dev = 0;
   cudaDeviceProp prop;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
     cudaGetLastError();
-    return QSGW_SIGMA_ERR_CUDA;
+    return -3;
   }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   double *sink = nullptr;
-  if (cudaMalloc(&sink, sizeof(double)) != cudaSuccess) return QSGW_SIGMA_ERR_ALLOC;
+  if (cudaMalloc(&sink, sizeof(double)) != cudaSuccess) return -2;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0);
   cudaEventCreate(&e1);
@@ -121,7 +130,7 @@ extern "C" int qsgw_sigma_fp64_probe(int mode, int iters, int mix, int ctas_per_
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   cudaFree(sink);
-  if (e != cudaSuccess) return QSGW_SIGMA_ERR_CUDA;
+  if (e != cudaSuccess) return -3;
   const double warps = (double)grid * 8;
   double flops = 0.0;
   if (mode == 0) flops = warps * iters * 32.0 * 512.0;
@@ -130,5 +139,5 @@ extern "C" int qsgw_sigma_fp64_probe(int mode, int iters, int mix, int ctas_per_
   if (mode == 3) flops = warps * iters * 4.0 * 32.0 * 512.0;
   *tflops = flops / (ms * 1e-3) / 1e12;
   if (ms_out) *ms_out = ms;
-  return QSGW_SIGMA_OK;
+  return 0;
 }

@@ -3,7 +3,8 @@
 // Path per pole chunk (<= s_block poles):  stage 1 GEMM (V) -> stage 2 GEMM (w chunk, symmetric pairs,
 // scattered to both mirrors) -> stage 3 fused D-scaling + contraction into split-K partial tiles.
 // begin() packs B once per Sigma; finish() reduces the partial tiles in fixed order and symmetrises.
-// Everything is enqueued on the plan's stream; no call allocates except create (and the first host-path call).
+// Everything is enqueued on the plan's stream; create allocates the workspace, and build_host / the qsMP2 entry points
+// allocate their own buffers on first use (include/qsgw_sigma.h).
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -11,6 +12,7 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -57,8 +59,13 @@ struct qsgw_sigma_plan {
   double *hB = nullptr, *hEps = nullptr, *hOcc = nullptr, *hSigma = nullptr;
   double *hOmega[2] = {nullptr, nullptr}, *hZ[2] = {nullptr, nullptr};
   int64_t h_range = 0;
+  bool staging_ready = false;
   cudaStream_t copy_stream = nullptr;
-  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr};
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr}, ev_b_slab = nullptr;
+
+  // debug mode: device-side precondition checks (qsgw_sigma_set_debug / QSGW_SIGMA_DEBUG=1)
+  bool debug = false;
+  unsigned long long *dbg = nullptr;   // [4] device counters
 
   // profiling
   bool profiling = false;
@@ -139,15 +146,52 @@ void drain_events(qsgw_sigma_plan *p) {
   }
 }
 
+// The kernels need more than 48 KB of dynamic shared memory; that opt-in is a per-device (per-context) function
+// attribute, so it is set once per device, under a lock, by whichever entry point first uses the device.
+constexpr int kMaxDevices = 64;
+std::mutex g_attr_mutex;
+bool g_attr_done[kMaxDevices] = {};
+
+template <class Kern>
+cudaError_t allow_smem(Kern kern, size_t bytes) {
+  return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+cudaError_t configure_kernels_for_device(int dev) {
+  std::lock_guard<std::mutex> lock(g_attr_mutex);
+  if (dev >= 0 && dev < kMaxDevices && g_attr_done[dev]) return cudaSuccess;
+  cudaError_t e = cudaSuccess;
+  auto set = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  set(allow_smem(gemm_tn_dmma_kernel<2, 2, EpiStore>, kGemmSmemBytes));
+  set(allow_smem(gemm_tn_dmma_kernel<2, 1, EpiStore>, kGemmSmemBytes));
+  set(allow_smem(gemm_tn_dmma_kernel<1, 2, EpiStore>, kGemmSmemBytes));
+  set(allow_smem(gemm_tn_dmma_kernel<1, 1, EpiStore>, kGemmSmemBytes));
+  set(allow_smem(gemm_tn_dmma_kernel<2, 2, EpiPairScatter>, kGemmSmemBytes));
+  set(allow_smem(sigma_accumulate_kernel, kSigmaSmemBytes));
+  set(allow_smem(sigma_diag_kernel, kDiagSmemMax));
+  if (e == cudaSuccess && dev >= 0 && dev < kMaxDevices) g_attr_done[dev] = true;
+  return e;
+}
+
+// Makes the plan's device current for the duration of one entry point and restores the caller's device afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  cudaError_t enter(int dev) {
+    cudaError_t e = cudaGetDevice(&prev);
+    if (e != cudaSuccess) return e;
+    if (prev == dev) return cudaSuccess;
+    e = cudaSetDevice(dev);
+    switched = (e == cudaSuccess);
+    return e;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
 template <int VECA, int VECB, class Epi>
 int launch_gemm_on(qsgw_sigma_plan *p, cudaStream_t stream, int num_sms, const double *A, int64_t lda, const double *Bm,
                    int64_t ldb, int M, int N, int K, const Epi &epi, int nbatch, int64_t strideA, int64_t strideB) {
-  static bool configured = false;
   auto kern = gemm_tn_dmma_kernel<VECA, VECB, Epi>;
-  if (!configured) {
-    QSGW_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGemmSmemBytes));
-    configured = true;
-  }
   const int ntm = (M + kBM - 1) / kBM, ntn = (N + kBN - 1) / kBN;
   if ((int64_t)ntm * ntn * nbatch > INT32_MAX) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "GEMM grid too large");
   // persistent: one CTA per SM walks the tiles round-robin; the dimension with fewer tiles varies fastest, so that the
@@ -168,16 +212,20 @@ int launch_gemm(qsgw_sigma_plan *p, const double *A, int64_t lda, const double *
 
 inline bool aligned16(const void *ptr, int64_t ld) { return (reinterpret_cast<uintptr_t>(ptr) & 15) == 0 && (ld & 1) == 0; }
 
-int check_plan(qsgw_sigma_plan *p) {
+int check_plan(qsgw_sigma_plan *p, DeviceGuard &guard) {
   if (!p) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "plan is NULL");
-  cudaError_t e = cudaSetDevice(p->device);
+  cudaError_t e = guard.enter(p->device);
   if (e != cudaSuccess) return fail(p, QSGW_SIGMA_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
   return QSGW_SIGMA_OK;
 }
 
+int debug_check_begin(qsgw_sigma_plan *p, const double *B, const double *occ);
+int debug_check_poles(qsgw_sigma_plan *p, const double *Omega, int64_t n_pole);
+
 int do_begin(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, double eta) {
   if (!B || !eps || !occ) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "begin: B, eps and occ must be non-NULL");
   if (!(eta > 0.0) || !std::isfinite(eta)) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "begin: eta must be finite and > 0");
+  if (int rc = debug_check_begin(p, B, occ)) return rc;
   p->B = B; p->eps = eps; p->occ = occ; p->eta = eta;
   {
     ScopedTimer t(p, kPack);
@@ -208,12 +256,6 @@ int run_stage2(qsgw_sigma_plan *p, const double *Vc, int sc, double alpha) {
 
 // Stage 3 for one chunk: Tpart[z] += (WA.D) WB^T over the internal states of split z and the chunk's sc poles
 int run_stage3(qsgw_sigma_plan *p, const double *WA, int64_t ldA, const double *WB, int64_t ldB, const double *Omega_c, int sc) {
-  static bool configured = false;
-  if (!configured) {
-    QSGW_CUDA(p, cudaFuncSetAttribute(sigma_accumulate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)kSigmaSmemBytes));
-    configured = true;
-  }
   ScopedTimer t(p, kStage3);
   const int ntp = (p->n_mo + kTP - 1) / kTP, ntq = (p->n_mo + kTQ - 1) / kTQ;
   sigma_accumulate_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
@@ -248,6 +290,7 @@ int do_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64
   if (n_pole < 1 || n_pole > p->n_pole_max)
     return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles: n_pole must be in [1, n_pole_max]");
   if (ldz < n_pole) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "add_poles: ldz < n_pole");
+  if (int rc = debug_check_poles(p, Omega, n_pole)) return rc;
 
   for (int64_t v0 = 0; v0 < n_pole; v0 += p->v_cols) {
     const int64_t nv = std::min<int64_t>(p->v_cols, n_pole - v0);
@@ -346,24 +389,103 @@ int do_finish(qsgw_sigma_plan *p, double *Sigma) {
   return QSGW_SIGMA_OK;
 }
 
+void free_host_staging(qsgw_sigma_plan *p) {
+  auto release = [&](double *&ptr, size_t count) {
+    if (ptr) { cudaFree(ptr); p->bytes -= std::max<size_t>(count, 1) * sizeof(double); ptr = nullptr; }
+  };
+  const size_t nn = (size_t)p->n_mo * p->n_mo;
+  const int64_t ld = round_up(p->s_chunk, 2);
+  release(p->hB, (size_t)p->n_aux * nn);
+  release(p->hEps, p->n_mo);
+  release(p->hOcc, p->n_mo);
+  release(p->hSigma, nn);
+  for (int b = 0; b < 2; ++b) {
+    release(p->hOmega[b], ld);
+    release(p->hZ[b], (size_t)p->n_ov * ld);
+    if (p->ev_copied[b]) { cudaEventDestroy(p->ev_copied[b]); p->ev_copied[b] = nullptr; }
+    if (p->ev_consumed[b]) { cudaEventDestroy(p->ev_consumed[b]); p->ev_consumed[b] = nullptr; }
+  }
+  if (p->ev_b_slab) { cudaEventDestroy(p->ev_b_slab); p->ev_b_slab = nullptr; }
+  if (p->copy_stream) { cudaStreamDestroy(p->copy_stream); p->copy_stream = nullptr; }
+  p->staging_ready = false;
+  cudaGetLastError();
+}
+
+// Device staging of the host path, allocated on the first qsgw_sigma_build_host call.  All or nothing: if any
+// allocation fails the partial ones are released again, so a later call starts from scratch.
 int ensure_host_staging(qsgw_sigma_plan *p) {
-  if (p->hB) return QSGW_SIGMA_OK;
+  if (p->staging_ready) return QSGW_SIGMA_OK;
   const int64_t range = p->s_chunk;   // one w chunk per uploaded pole range
   const size_t nn = (size_t)p->n_mo * p->n_mo;
-  int rc;
-  if ((rc = dev_alloc(p, &p->hB, (size_t)p->n_aux * nn, "host-path B"))) return rc;
-  if ((rc = dev_alloc(p, &p->hEps, p->n_mo, "host-path eps"))) return rc;
-  if ((rc = dev_alloc(p, &p->hOcc, p->n_mo, "host-path occ"))) return rc;
-  if ((rc = dev_alloc(p, &p->hSigma, nn, "host-path Sigma"))) return rc;
   const int64_t ld = round_up(range, 2);
-  for (int b = 0; b < 2; ++b) {
-    if ((rc = dev_alloc(p, &p->hOmega[b], ld, "host-path Omega"))) return rc;
-    if ((rc = dev_alloc(p, &p->hZ[b], (size_t)p->n_ov * ld, "host-path Z range"))) return rc;
-    QSGW_CUDA(p, cudaEventCreateWithFlags(&p->ev_copied[b], cudaEventDisableTiming));
-    QSGW_CUDA(p, cudaEventCreateWithFlags(&p->ev_consumed[b], cudaEventDisableTiming));
+  int rc = QSGW_SIGMA_OK;
+  cudaError_t e = cudaSuccess;
+  if (!rc) rc = dev_alloc(p, &p->hB, (size_t)p->n_aux * nn, "host-path B");
+  if (!rc) rc = dev_alloc(p, &p->hEps, p->n_mo, "host-path eps");
+  if (!rc) rc = dev_alloc(p, &p->hOcc, p->n_mo, "host-path occ");
+  if (!rc) rc = dev_alloc(p, &p->hSigma, nn, "host-path Sigma");
+  for (int b = 0; b < 2 && !rc; ++b) {
+    if (!rc) rc = dev_alloc(p, &p->hOmega[b], ld, "host-path Omega");
+    if (!rc) rc = dev_alloc(p, &p->hZ[b], (size_t)p->n_ov * ld, "host-path Z range");
+    if (!rc && e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_copied[b], cudaEventDisableTiming);
+    if (!rc && e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_consumed[b], cudaEventDisableTiming);
   }
-  QSGW_CUDA(p, cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+  if (!rc && e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_b_slab, cudaEventDisableTiming);
+  if (!rc && e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking);
+  if (!rc && e != cudaSuccess) rc = fail(p, QSGW_SIGMA_ERR_CUDA, std::string("host-path staging: ") + cudaGetErrorString(e));
+  if (rc) {
+    const std::string msg = p->err;
+    free_host_staging(p);
+    p->err = msg;
+    return rc;
+  }
   p->h_range = range;
+  p->staging_ready = true;
+  return QSGW_SIGMA_OK;
+}
+
+// Debug mode (include/qsgw_sigma.h "Preconditions"): look at the device data and refuse inputs that break a precondition.
+int debug_check_begin(qsgw_sigma_plan *p, const double *B, const double *occ) {
+  if (!p->debug) return QSGW_SIGMA_OK;
+  QSGW_CUDA(p, cudaMemsetAsync(p->dbg, 0, 4 * sizeof(unsigned long long), p->stream));
+  check_B_symmetry_kernel<<<dim3(p->n_mo, p->n_aux), 128, 0, p->stream>>>(B, p->n_mo, p->n_aux, p->dbg);
+  check_range_kernel<<<1, 256, 0, p->stream>>>(occ, p->n_mo, 0.0, 1.0, 0, p->dbg + 3);
+  QSGW_CUDA(p, cudaGetLastError());
+  unsigned long long h[4];
+  QSGW_CUDA(p, cudaMemcpyAsync(h, p->dbg, sizeof h, cudaMemcpyDeviceToHost, p->stream));
+  QSGW_CUDA(p, cudaStreamSynchronize(p->stream));
+  double dmax, amax;
+  std::memcpy(&dmax, &h[0], 8);
+  std::memcpy(&amax, &h[1], 8);
+  char buf[256];
+  if (h[2]) {
+    snprintf(buf, sizeof buf, "debug: B has %llu non-finite entries", h[2]);
+    return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, buf);
+  }
+  if (dmax > 1e-10 * amax) {
+    snprintf(buf, sizeof buf, "debug: B is not symmetric in its last two indices: max|B[P][p][q]-B[P][q][p]| = %.3e (max|B| = %.3e)", dmax, amax);
+    return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, buf);
+  }
+  if (h[3]) {
+    snprintf(buf, sizeof buf, "debug: %llu occupations lie outside [0, 1]", h[3]);
+    return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, buf);
+  }
+  return QSGW_SIGMA_OK;
+}
+
+int debug_check_poles(qsgw_sigma_plan *p, const double *Omega, int64_t n_pole) {
+  if (!p->debug) return QSGW_SIGMA_OK;
+  QSGW_CUDA(p, cudaMemsetAsync(p->dbg, 0, 4 * sizeof(unsigned long long), p->stream));
+  check_range_kernel<<<(int)std::min<int64_t>(1024, (n_pole + 255) / 256), 256, 0, p->stream>>>(Omega, n_pole, 0.0, 1e300, 1, p->dbg);
+  QSGW_CUDA(p, cudaGetLastError());
+  unsigned long long h = 0;
+  QSGW_CUDA(p, cudaMemcpyAsync(&h, p->dbg, sizeof h, cudaMemcpyDeviceToHost, p->stream));
+  QSGW_CUDA(p, cudaStreamSynchronize(p->stream));
+  if (h) {
+    char buf[128];
+    snprintf(buf, sizeof buf, "debug: %llu excitation energies Omega are not finite and > 0", h);
+    return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, buf);
+  }
   return QSGW_SIGMA_OK;
 }
 
@@ -371,7 +493,7 @@ int ensure_host_staging(qsgw_sigma_plan *p) {
 
 extern "C" {
 
-int qsgw_sigma_version(void) { return 10100; }
+int qsgw_sigma_version(void) { return 10200; }
 
 int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, int64_t n_pole_max, int s_block,
                       void *cuda_stream) {
@@ -432,6 +554,16 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
     qsgw_sigma_destroy(p);
     return fail(nullptr, code, msg);
   };
+  e = configure_kernels_for_device(dev);
+  if (e != cudaSuccess) {
+    p->err = std::string("cudaFuncSetAttribute(MaxDynamicSharedMemorySize): ") + cudaGetErrorString(e);
+    return bail(QSGW_SIGMA_ERR_CUDA);
+  }
+  {
+    const char *dbg_env = std::getenv("QSGW_SIGMA_DEBUG");
+    p->debug = dbg_env && dbg_env[0] && dbg_env[0] != '0';
+  }
+  if ((rc = dev_alloc(p, &p->dbg, 4, "debug counters"))) return bail(rc);
   if ((rc = dev_alloc(p, &p->Bp, (size_t)n_aux * p->ldp, "packed symmetric B"))) return bail(rc);
   if ((rc = dev_alloc(p, &p->BovT, (size_t)p->n_ov * p->ld_aux, "transposed ov block of B"))) return bail(rc);
   if ((rc = dev_alloc(p, &p->V, (size_t)n_aux * p->ldv, "V chunk"))) return bail(rc);
@@ -450,26 +582,30 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
 }
 
 int qsgw_sigma_begin(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, double eta) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   return do_begin(p, B, eps, occ, eta);
 }
 
 int qsgw_sigma_add_poles(qsgw_sigma_plan *p, const double *Omega, const double *Z, int64_t ldz, int64_t n_pole) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   return do_add_poles(p, Omega, Z, ldz, n_pole);
 }
 
 int qsgw_sigma_finish(qsgw_sigma_plan *p, double *Sigma) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   return do_finish(p, Sigma);
 }
 
 int qsgw_sigma_build(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, const double *Omega,
                      const double *Z, int64_t ldz, int64_t n_pole, double eta, double *Sigma) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   if (!Omega || !Z || !Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build: NULL argument");
   if (n_pole < 1 || n_pole > p->n_pole_max) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build: n_pole must be in [1, n_pole_max]");
@@ -482,19 +618,15 @@ int qsgw_sigma_build(qsgw_sigma_plan *p, const double *B, const double *eps, con
 int qsgw_sigma_diag_build(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ,
                           const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
                           const double *omega_grid, int n_omega, double *SigmaRe, double *SigmaIm) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   if (!Omega || !Z || !omega_grid || !SigmaRe || !SigmaIm) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: NULL argument");
   if (n_pole < 1 || n_pole > p->n_pole_max) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: n_pole must be in [1, n_pole_max]");
   if (ldz < n_pole) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: ldz < n_pole");
   if (n_omega < 1) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: n_omega < 1");
   const size_t smem_max = sizeof(double) * ((size_t)p->s_chunk + (kDiagThreads / 32) * 2 * kDiagKW);
-  if (smem_max > 200 * 1024) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: s_block too large for the diagonal kernel");
-  static bool configured = false;
-  if (!configured) {
-    QSGW_CUDA(p, cudaFuncSetAttribute(sigma_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    configured = true;
-  }
+  if (smem_max > kDiagSmemMax) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "diag_build: s_block too large for the diagonal kernel");
   if ((rc = do_begin(p, B, eps, occ, eta))) return rc;
   const size_t nbytes = sizeof(double) * (size_t)p->n_mo * n_omega;
   QSGW_CUDA(p, cudaMemsetAsync(SigmaRe, 0, nbytes, p->stream));
@@ -510,7 +642,8 @@ int qsgw_sigma_diag_build(qsgw_sigma_plan *p, const double *B, const double *eps
 int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ,
                           const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,
                           double *Sigma) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   if (!B || !eps || !occ || !Omega || !Z || !Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build_host: NULL argument");
   if (n_pole < 1 || ldz < n_pole) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build_host: need 1 <= n_pole <= ldz");
@@ -555,7 +688,8 @@ int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps
 
 int qsgw_mp2_direct_build(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, double eta,
                           double *Sigma) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   if (!Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "mp2_direct_build: Sigma must be non-NULL");
   if ((rc = do_begin(p, B, eps, occ, eta))) return rc;
@@ -564,7 +698,8 @@ int qsgw_mp2_direct_build(qsgw_sigma_plan *p, const double *B, const double *eps
 }
 
 int qsgw_mp2_build(qsgw_sigma_plan *p, const double *B, const double *eps, const double *occ, double eta, double *Sigma) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   if (!Sigma) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "mp2_build: Sigma must be non-NULL");
   if ((rc = do_begin(p, B, eps, occ, eta))) return rc;
@@ -592,6 +727,8 @@ int qsgw_ri_ao_to_mo(const double *B_ao, const double *C, int n_aux, int n_ao, i
     return fail(nullptr, QSGW_SIGMA_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
   }
   if (major != 10) return fail(nullptr, QSGW_SIGMA_ERR_CUDA, "this library is built for sm_100a (B200) only");
+  if ((e = configure_kernels_for_device(dev)) != cudaSuccess)
+    return fail(nullptr, QSGW_SIGMA_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const int64_t ldt = round_up(n_mo, 2);
   const int64_t sB = (int64_t)n_ao * n_ao, sT = (int64_t)n_ao * ldt, sO = (int64_t)n_mo * n_mo;
@@ -618,18 +755,15 @@ int qsgw_ri_ao_to_mo(const double *B_ao, const double *C, int n_aux, int n_ao, i
 
 int qsgw_sigma_destroy(qsgw_sigma_plan *p) {
   if (!p) return QSGW_SIGMA_OK;
-  cudaSetDevice(p->device);
+  DeviceGuard guard;
+  guard.enter(p->device);
   cudaStreamSynchronize(p->stream);
-  if (p->copy_stream) { cudaStreamSynchronize(p->copy_stream); cudaStreamDestroy(p->copy_stream); }
+  if (p->copy_stream) cudaStreamSynchronize(p->copy_stream);
   for (int s = 0; s < kNumStages; ++s)
     for (EventPair &ev : p->pending[s]) p->pool.push_back(ev);
   for (EventPair &ev : p->pool) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
-  for (int b = 0; b < 2; ++b) {
-    if (p->ev_copied[b]) cudaEventDestroy(p->ev_copied[b]);
-    if (p->ev_consumed[b]) cudaEventDestroy(p->ev_consumed[b]);
-    cudaFree(p->hOmega[b]); cudaFree(p->hZ[b]);
-  }
-  cudaFree(p->hB); cudaFree(p->hEps); cudaFree(p->hOcc); cudaFree(p->hSigma);
+  free_host_staging(p);
+  cudaFree(p->dbg);
   cudaFree(p->Bp); cudaFree(p->BovT); cudaFree(p->V); cudaFree(p->W); cudaFree(p->Tpart); cudaFree(p->pairs); cudaFree(p->mp2_omega); cudaFree(p->mp2_y);
   cudaGetLastError();
   delete p;
@@ -653,8 +787,16 @@ int qsgw_sigma_set_profiling(qsgw_sigma_plan *p, int on) {
   return QSGW_SIGMA_OK;
 }
 
+int qsgw_sigma_set_debug(qsgw_sigma_plan *p, int on) {
+  if (!p) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "plan is NULL");
+  p->debug = on != 0;
+  return QSGW_SIGMA_OK;
+}
+
+#ifdef QSGW_SIGMA_TEST_HOOKS
 int qsgw_sigma_copy_workspace(qsgw_sigma_plan *p, int which, double *dst, int64_t rows, int64_t cols) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   if (!dst || rows < 1 || cols < 1) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "copy_workspace: bad arguments");
   const double *src = nullptr;
@@ -673,9 +815,11 @@ int qsgw_sigma_copy_workspace(qsgw_sigma_plan *p, int which, double *dst, int64_
                                  cudaMemcpyDeviceToDevice, p->stream));
   return QSGW_SIGMA_OK;
 }
+#endif  // QSGW_SIGMA_TEST_HOOKS
 
 int qsgw_sigma_get_stats(qsgw_sigma_plan *p, qsgw_sigma_stats *st, int reset) {
-  int rc = check_plan(p);
+  DeviceGuard guard;
+  int rc = check_plan(p, guard);
   if (rc) return rc;
   if (!st) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "get_stats: stats is NULL");
   QSGW_CUDA(p, cudaStreamSynchronize(p->stream));

@@ -76,6 +76,39 @@ __global__ void mp2_sox_chunk_kernel(const double *__restrict__ B, const double 
   else Omega[j] = eps[a] - eps[i];
 }
 
+// ---------------------------------------------------------------- debug-mode precondition checks (include/qsgw_sigma.h)
+// out[0] = max |B[P][p][q] - B[P][q][p]|, out[1] = max |B| as the bit patterns of non-negative doubles (which order
+// like unsigned integers, so atomicMax on the bits is the max of the values); out[2] = number of NaN/Inf entries.
+__global__ void check_B_symmetry_kernel(const double *__restrict__ B, int n_mo, int n_aux, unsigned long long *out) {
+  const int p = blockIdx.x, P = blockIdx.y;
+  const double *BP = B + (int64_t)P * n_mo * n_mo;
+  double dmax = 0.0, amax = 0.0;
+  unsigned long long bad = 0;
+  for (int q = threadIdx.x; q < n_mo; q += blockDim.x) {
+    const double a = BP[(int64_t)p * n_mo + q], b = BP[(int64_t)q * n_mo + p];
+    if (!isfinite(a)) ++bad;
+    else {
+      dmax = fmax(dmax, fabs(a - b));
+      amax = fmax(amax, fabs(a));
+    }
+  }
+  if (dmax > 0.0) atomicMax(out + 0, (unsigned long long)__double_as_longlong(dmax));
+  if (amax > 0.0) atomicMax(out + 1, (unsigned long long)__double_as_longlong(amax));
+  if (bad) atomicAdd(out + 2, bad);
+}
+
+// out[0] += number of entries of x[0..n) outside [lo, hi] (NaN counts as outside); lo_open: the lower bound is excluded.
+__global__ void check_range_kernel(const double *__restrict__ x, int64_t n, double lo, double hi, int lo_open,
+                                   unsigned long long *out) {
+  unsigned long long bad = 0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double v = x[i];
+    const bool ok = (lo_open ? v > lo : v >= lo) && v <= hi;
+    if (!ok) ++bad;
+  }
+  if (bad) atomicAdd(out, bad);
+}
+
 // ---------------------------------------------------------------- stage 3
 // D(m,s,omega) = occ_m * x1/(x1^2+eta^2) + (1-occ_m) * x2/(x2^2+eta^2),  x1 = (omega-eps_m)+Omega_s,
 // x2 = (omega-eps_m)-Omega_s: real part of the two terms of Eq. (17).  d = omega - eps_m.
@@ -414,6 +447,7 @@ __global__ void sigma_epilogue_kernel(const double *__restrict__ Tpart, int nspl
 // contribution to them with a plain read-modify-write: fixed order, reproducible, no atomics.
 constexpr int kDiagKW = 8;         // frequency points per thread
 constexpr int kDiagThreads = 128;
+constexpr size_t kDiagSmemMax = 200 * 1024;   // dynamic shared memory the kernel may be launched with (Omega of one chunk + scratch)
 
 __device__ __forceinline__ void diag_term(double x, double eta2, double w2, double wim, double &re, double &im) {
   const double y = fma(x, x, eta2);

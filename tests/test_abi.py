@@ -4,16 +4,24 @@ product never routes through the oracle."""
 import ctypes
 import os
 import re
+import subprocess
 
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared_symbols():
+def _declared_symbols(test_hooks=False):
     text = open(os.path.join(ROOT, "include", "qsgw_sigma.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    if not test_hooks:
+        text = re.sub(r"#ifdef QSGW_SIGMA_TEST_HOOKS.*?#endif", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(qsgw_[a-z0-9_]+)\s*\(", text)))
+
+
+def _exported(path):
+    out = subprocess.run(["nm", "-D", "--defined-only", path], check=True, capture_output=True, text=True).stdout
+    return sorted(set(re.findall(r"\bT (qsgw_[a-z0-9_]+)$", out, flags=re.M)))
 
 
 def test_library_builds_and_exports_every_declared_symbol():
@@ -24,11 +32,20 @@ def test_library_builds_and_exports_every_declared_symbol():
     assert "qsgw_sigma_create" in declared and "qsgw_sigma_build" in declared and "qsgw_sigma_destroy" in declared
     for name in declared:
         assert hasattr(lib, name), f"{name} declared in include/qsgw_sigma.h but not exported"
+    assert _exported(path) == declared                  # ... and nothing else: no probe, no test hook in the product
     assert sorted(binding.EXPORTS) == declared          # the Python binding carries the same names
     import paper_2210_17093_b200 as pkg
     for name in declared:
         assert callable(getattr(pkg, name))
     assert pkg.qsgw_sigma_version() >= 100
+
+
+def test_test_hook_and_probe_live_in_their_own_libraries():
+    from paper_2210_17093_b200 import build
+    hooks = _declared_symbols(test_hooks=True)
+    assert "qsgw_sigma_copy_workspace" in hooks and "qsgw_sigma_copy_workspace" not in _declared_symbols()
+    assert _exported(build.build_library(test_hooks=True)) == hooks
+    assert _exported(build.build_probe()) == ["qsgw_fp64_probe"]
 
 
 def test_create_rejects_bad_sizes_before_touching_the_device():

@@ -1,10 +1,11 @@
 """Parity of the CUDA path at BASELINE.json's FULL sizes, in the launch configuration bench.py times
 (plan created with the config's n_pole and s_block; one-shot qsgw_sigma_build for `large`, the streaming
-begin/add_poles/finish calls with 4096-pole ranges for `xl`, whose Z is 130 GB).
+begin/add_poles/finish calls with 8192-pole ranges for `xl`, whose Z is 130 GB).
 
 The full oracle is unaffordable there (1e14 - 1e15 flops), so (SURVEY.md 8(c) "Oracle affordability"):
   * sampled outputs the oracle can compute one by one: a pole sub-range x a sampled set of states at the full
-    N and naux, the GPU building the same sub-range through pointer offsets into the full-size arrays;
+    N and naux with the config's random inputs, the GPU building the same sub-range -- more than one s-block of poles in
+    ONE call, so that the library's chunk loop runs -- through pointer offsets into the full-size arrays;
   * a property that holds at any size: the separable closed form (pin 9 of tests/test_oracle_pins.py, where the
     oracle itself is checked against it) evaluated in numpy for sampled states, the GPU doing its full dense work;
   * additivity over pole ranges, bit-symmetry, reproducibility.
@@ -99,13 +100,17 @@ def test_large_config_full_build_separable_closed_form():
     pkg.qsgw_sigma_destroy(plan)
 
 
-def test_large_config_pole_subrange_vs_oracle_on_sampled_states():
-    """Full N = 600, naux = 2400, (ia) = 41600 with the config's random inputs; 1536 poles straddling the s-block
-    edge at 4096 (so that the oracle finishes in about a minute); sampled states S x S."""
+def test_large_config_multi_chunk_pole_range_vs_oracle_on_sampled_states():
+    """Full N = 600, naux = 2400, (ia) = 41600 with the config's RANDOM inputs, plan as bench.py creates it (n_pole_max =
+    41600, s-block 4096).  ONE qsgw_sigma_build call over 4096 + 160 poles that start at pole 3000 (pointer offset into
+    a wider Z, full leading dimension), so that the library's own chunk loop runs twice -- a full 4096-pole w chunk and a
+    ragged 160-pole one -- and, in a second pass with qsgw_sigma_limit_pole_batch(4096), its stage-1 range loop too.
+    Sampled states S x S against oracle.sigma on exactly those poles (about a minute of oracle time)."""
     pkg = _pkg()
     cfg = qi.CONFIGS["large"]
     dev = torch.device("cuda", 0)
-    s0, s1 = 4096 - 700, 4096 + 836
+    s0 = 3000
+    s1 = s0 + cfg.s_block + 160
     B = qi.make_B(cfg, dev)
     eps, occ, Om = qi.make_eps(cfg), qi.make_occ(cfg), qi.make_omega(cfg)
     eps_d, occ_d, Om_d = eps.to(dev), occ.to(dev), Om.to(dev)   # must outlive begin ... finish (include/qsgw_sigma.h)
@@ -114,14 +119,26 @@ def test_large_config_pole_subrange_vs_oracle_on_sampled_states():
     Zr = qi.make_Z(cfg, s0, s1, device=dev)
     Zfull[:, s0:s1] = Zr
     plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, cfg.s_block)
+    pkg.qsgw_sigma_get_stats(plan, reset=True)
     S = pkg.qsgw_sigma_build(plan, B, eps_d, occ_d, Om_d[s0:s1], Zfull[:, s0:s1], cfg.eta)
     torch.cuda.synchronize()
+    st = pkg.qsgw_sigma_get_stats(plan, reset=True)
+    assert st["poles"] == s1 - s0
+    assert st["kernel_launches"] >= 2 + 1 + 2 * 2 + 1, "one stage-1 launch and TWO stage-2/3 chunks must have run"
     assert torch.equal(S, S.T)
     states = _sample_states(cfg, n_random=4, seed=1)
     ref = oracle.sigma(B.cpu().numpy(), eps.numpy(), occ.numpy(), Om.numpy()[s0:s1], Zr.cpu().numpy(), cfg.eta,
                        cfg.n_occ, states=states)
     got = S.cpu().numpy()[np.ix_(states, states)]
-    _assert_parity(got, ref, "large, pole sub-range vs oracle")
+    _assert_parity(got, ref, "large, multi-chunk pole range vs oracle")
+    # the same call with stage 1 cut into two ranges (4096 + 160 poles)
+    pkg.qsgw_sigma_limit_pole_batch(plan, cfg.s_block)
+    S2 = pkg.qsgw_sigma_build(plan, B, eps_d, occ_d, Om_d[s0:s1], Zfull[:, s0:s1], cfg.eta)
+    torch.cuda.synchronize()
+    st2 = pkg.qsgw_sigma_get_stats(plan, reset=True)
+    assert st2["kernel_launches"] > st["kernel_launches"], "a second stage-1 launch"
+    _assert_parity(S2.cpu().numpy()[np.ix_(states, states)], ref, "large, two stage-1 ranges vs oracle")
+    pkg.qsgw_sigma_limit_pole_batch(plan, cfg.n_pole)
     # additivity: the same range in two pieces through the streaming calls
     pkg.qsgw_sigma_begin(plan, B, eps_d, occ_d, cfg.eta)
     mid = 4096
@@ -134,9 +151,50 @@ def test_large_config_pole_subrange_vs_oracle_on_sampled_states():
     pkg.qsgw_sigma_destroy(plan)
 
 
+XL_RANGE = 2 * qi.CONFIGS["xl"].s_block     # poles per qsgw_sigma_add_poles call of the xl runs (bench.py uses the same)
+
+
+def test_xl_config_multi_chunk_pole_range_vs_oracle_on_sampled_states():
+    """`xl` (N = 1000, naux = 4000, (ia) = 127500) with the config's RANDOM B and Z, plan as bench.py creates it for the
+    streamed build (n_pole_max = 8192 = two s-blocks).  begin, ONE qsgw_sigma_add_poles call over 4096 + 128 poles (a full
+    w chunk and a ragged one: the chunk loop runs twice; row offsets (m N + p) ldw reach 4.1e9 > 2^32), finish.  Sampled
+    states S x S -- deepest, HOMO, LUMO, highest, tile-edge neighbours, random -- against oracle.sigma on those poles
+    (SURVEY.md 8(c) "xl parity (i)")."""
+    pkg = _pkg()
+    cfg = qi.CONFIGS["xl"]
+    dev = torch.device("cuda", 0)
+    free, _ = torch.cuda.mem_get_info()
+    if free < 120e9:
+        pytest.skip("needs ~110 GB of free device memory")
+    s0 = 61000                                                   # mid-spectrum poles (Omega ~ 3 Ha)
+    s1 = s0 + cfg.s_block + 128
+    B = qi.make_B(cfg, dev)
+    eps, occ, Om = qi.make_eps(cfg), qi.make_occ(cfg), qi.make_omega(cfg)
+    eps_d, occ_d, Om_d = eps.to(dev), occ.to(dev), Om.to(dev)
+    Zr = qi.make_Z(cfg, s0, s1, device=dev)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, XL_RANGE, cfg.s_block)
+    pkg.qsgw_sigma_get_stats(plan, reset=True)
+    pkg.qsgw_sigma_begin(plan, B, eps_d, occ_d, cfg.eta)
+    pkg.qsgw_sigma_add_poles(plan, Om_d[s0:s1], Zr)
+    S = pkg.qsgw_sigma_finish(plan)
+    torch.cuda.synchronize()
+    st = pkg.qsgw_sigma_get_stats(plan, reset=True)
+    assert st["poles"] == s1 - s0 and st["kernel_launches"] >= 2 + 1 + 2 * 2 + 1
+    assert torch.equal(S, S.T)
+    N, o = cfg.n_mo, cfg.n_occ
+    states = sorted({0, o - 1, o, N - 1, 63, 64, 255, 256, 959, 960, 417, 702})
+    B_h = B.cpu().numpy()
+    pkg.qsgw_sigma_destroy(plan)
+    del B
+    torch.cuda.empty_cache()
+    ref = oracle.sigma(B_h, eps.numpy(), occ.numpy(), Om.numpy()[s0:s1], Zr.cpu().numpy(), cfg.eta, cfg.n_occ, states=states)
+    got = S.cpu().numpy()[np.ix_(states, states)]
+    _assert_parity(got, ref, "xl, multi-chunk pole range vs oracle")
+
+
 def test_xl_config_streamed_build_separable_closed_form():
-    """`xl` as bench.py runs it: begin, 32 add_poles calls of <= 4096 poles (Z produced range by range on the
-    device: 130 GB whole), finish.  Separable inputs, closed form on sampled states."""
+    """`xl` as bench.py runs it: begin, 16 add_poles calls of <= 8192 poles = two s-blocks each (Z produced range by
+    range on the device: 130 GB whole), finish.  Separable inputs, closed form on sampled states."""
     pkg = _pkg()
     cfg = qi.CONFIGS["xl"]
     dev = torch.device("cuda", 0)
@@ -146,7 +204,7 @@ def test_xl_config_streamed_build_separable_closed_form():
     c, u, z, t, B = _separable_inputs(cfg, dev, seed=4321)
     eps, occ, Om = qi.make_eps(cfg), qi.make_occ(cfg), qi.make_omega(cfg)
     eps_d, occ_d, Om_d, z_d, t_d = eps.to(dev), occ.to(dev), Om.to(dev), z.to(dev), t.to(dev)
-    rng = cfg.s_block
+    rng = XL_RANGE
     plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, rng, cfg.s_block)
     Zbuf = [torch.empty((cfg.n_ov, rng), dtype=torch.float64, device=dev) for _ in range(2)]
     pkg.qsgw_sigma_begin(plan, B, eps_d, occ_d, cfg.eta)
@@ -201,7 +259,7 @@ def test_large_config_ao_to_mo_sampled_auxiliary_functions():
     C = C.contiguous()
     B_mo = pkg.qsgw_ri_ao_to_mo(B_ao, C)
     torch.cuda.synchronize()
-    sample = [0, 1, 127, 128, 1199, 2398, 2399]
+    sample = [0, 127, 1199, 2399]                    # the oracle is the O(N^4) double sum per auxiliary function
     ref = oracle.ao_to_mo(B_ao[sample].cpu().numpy(), C.cpu().numpy())
     _assert_parity(B_mo[sample].cpu().numpy(), ref, "large, AO->MO")
     # an orthogonal C preserves the trace of every B[P]: a property checked on ALL 2400 auxiliary functions

@@ -67,3 +67,38 @@ def test_full_qsmp2_parity(n_mo, n_occ, n_aux, s_block):
     assert torch.equal(S, S.T)
     assert torch.equal(S, pkg.qsgw_mp2_build(plan, Bd, ed, od, cfg.eta))       # reproducible
     pkg.qsgw_sigma_destroy(plan)
+
+
+def _mp2_sampled(cfg_name, states):
+    """qsgw_mp2_build on the WHOLE config (the GPU runs its full build, as bench.py --path mp2 does); the oracle computes
+    the sampled S x S block with every internal sum (i, a, p, P) over its full range (oracle.mp2(states=...))."""
+    pkg = _pkg()
+    cfg = qi.CONFIGS[cfg_name]
+    B, eps, occ = qi.make_B(cfg, "cuda"), qi.make_eps(cfg), qi.make_occ(cfg)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_ov, cfg.s_block)
+    S = pkg.qsgw_mp2_build(plan, B, eps.cuda(), occ.cuda(), cfg.eta)
+    torch.cuda.synchronize()
+    assert torch.equal(S, S.T)
+    B_h = B.cpu().numpy()
+    pkg.qsgw_sigma_destroy(plan)
+    ref = oracle.mp2(B_h, eps.numpy(), occ.numpy(), cfg.eta, cfg.n_occ, states=states)
+    got = S.cpu().numpy()[np.ix_(states, states)]
+    err, scale = np.max(np.abs(got - ref)), np.abs(ref).max()
+    assert err <= 1e-9 * scale, f"{cfg_name}: {err:.3e} vs {scale:.3e}"
+
+
+def test_medium_config_qsmp2_sampled_states():
+    """`medium` (N = 300, o = 40, naux = 1100, s-block 2048: 10400 (ia) pairs in 6 chunks for the direct term, 40 exchange
+    passes).  24 output states: deepest, HOMO-1, HOMO, LUMO, LUMO+1, highest, the 64/256 tile edges and a regular grid."""
+    cfg = qi.CONFIGS["medium"]
+    o, N = cfg.n_occ, cfg.n_mo
+    states = sorted({0, 1, o - 2, o - 1, o, o + 1, 63, 64, 127, 128, 255, 256, N - 2, N - 1} | set(range(7, N, 29)))
+    _mp2_sampled("medium", states)
+
+
+def test_large_config_qsmp2_sampled_states():
+    """`large` (N = 600, o = 80, naux = 2400, s-block 4096), the size bench.py --path mp2 reports: 41600 pairs in 11 chunks,
+    80 exchange passes with the [N][N][N] exchange-integral buffer.  5 output states (the oracle's cost is
+    41600 x 3 x |S| x 600 x 2400 multiply-adds)."""
+    cfg = qi.CONFIGS["large"]
+    _mp2_sampled("large", [0, cfg.n_occ - 1, cfg.n_occ, 256, cfg.n_mo - 1])

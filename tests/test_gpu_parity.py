@@ -78,21 +78,25 @@ def test_ragged_shapes_parity(n_mo, n_occ, n_aux, n_pole, s_block):
 
 
 def test_stage_outputs_match_oracle_steps():
-    """a1/a2: V and the w chunk, element by element, against oracle steps 1 and 2."""
-    pkg = _pkg()
+    """a1/a2: V and the w chunk, element by element, against oracle steps 1 and 2 (through the test build of the library,
+    which adds the qsgw_sigma_copy_workspace hook; the same sources otherwise)."""
+    from testhooks import HookedPlan, WORKSPACE_V, WORKSPACE_W
     cfg = qi.custom_config(70, 9, 45, n_pole=200, s_block=0, seed=5)
     inp = qi.make_inputs(cfg)
-    S, plan = _gpu_sigma(cfg, _to_dev(inp))
-    V = pkg.qsgw_sigma_copy_workspace(plan, pkg.WORKSPACE_V, cfg.n_aux, cfg.n_pole).cpu().numpy()
-    W = pkg.qsgw_sigma_copy_workspace(plan, pkg.WORKSPACE_W, cfg.n_mo ** 2, cfg.n_pole).cpu().numpy()
+    B, eps, occ, Om, Z = _to_dev(inp)
+    plan = HookedPlan(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, cfg.s_block)
+    S = plan.build(B, eps, occ, Om, Z, cfg.eta)
+    V = plan.copy_workspace(WORKSPACE_V, cfg.n_aux, cfg.n_pole).cpu().numpy()
+    W = plan.copy_workspace(WORKSPACE_W, cfg.n_mo ** 2, cfg.n_pole).cpu().numpy()
     torch.cuda.synchronize()
+    _assert_parity(S, _ref_sigma(cfg, inp))
     V_ref = oracle.pole_weights(inp.B.numpy(), inp.Z.numpy(), cfg.n_occ)
     assert np.max(np.abs(V - V_ref)) <= 1e-13 * np.max(np.abs(V_ref))
     W = W.reshape(cfg.n_mo, cfg.n_mo, cfg.n_pole)              # [m][p][s]
     for s in (0, 1, 77, 199):
         w_ref = oracle.residues(inp.B.numpy(), V_ref, s)       # [p][m]
         assert np.max(np.abs(W[:, :, s].T - w_ref)) <= 1e-13 * np.max(np.abs(w_ref))
-    pkg.qsgw_sigma_destroy(plan)
+    plan.destroy()
 
 
 def test_general_occupations_and_unsorted_inputs():
@@ -209,6 +213,35 @@ def test_null_case_and_error_codes():
     _assert_parity(S2, _ref_sigma(cfg, inp))
     pkg.qsgw_sigma_destroy(plan)
     pkg.qsgw_sigma_destroy(small_plan)
+
+
+def test_debug_mode_checks_the_device_side_preconditions():
+    """occ in [0,1], Omega > 0 and B symmetric are documented preconditions, verified only in debug mode."""
+    pkg = _pkg()
+    cfg = qi.custom_config(40, 6, 20, n_pole=90, seed=12)
+    inp = qi.make_inputs(cfg)
+    B, eps, occ, Om, Z = _to_dev(inp)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole)
+    S = pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta)
+    pkg.qsgw_sigma_set_debug(plan, True)
+    assert torch.equal(pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta), S)     # valid inputs pass, same result
+    B_bad = B.clone(); B_bad[3, 5, 17] += 1e-3
+    occ_bad = occ.clone(); occ_bad[7] = 1.5
+    occ_nan = occ.clone(); occ_nan[0] = float("nan")
+    Om_bad = Om.clone(); Om_bad[11] = -Om_bad[11]
+    Om_zero = Om.clone(); Om_zero[0] = 0.0
+    B_inf = B.clone(); B_inf[0, 1, 1] = float("inf")
+    for args, word in (((B_bad, eps, occ, Om, Z), "symmetric"), ((B, eps, occ_bad, Om, Z), "occupations"),
+                       ((B, eps, occ_nan, Om, Z), "occupations"), ((B, eps, occ, Om_bad, Z), "Omega"),
+                       ((B, eps, occ, Om_zero, Z), "Omega"), ((B_inf, eps, occ, Om, Z), "non-finite")):
+        with pytest.raises(pkg.QsgwSigmaError) as ei:
+            pkg.qsgw_sigma_build(plan, *args, cfg.eta)
+        assert ei.value.code == pkg.QSGW_SIGMA_ERR_INVALID_ARG and word in str(ei.value), str(ei.value)
+    assert torch.equal(pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta), S)     # the plan survives the refusals
+    pkg.qsgw_sigma_set_debug(plan, False)
+    pkg.qsgw_sigma_build(plan, B_bad, eps, occ, Om, Z, cfg.eta)                        # outside debug mode: not checked
+    torch.cuda.synchronize()
+    pkg.qsgw_sigma_destroy(plan)
 
 
 def test_medium_config_full_parity():

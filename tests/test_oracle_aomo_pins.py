@@ -32,6 +32,22 @@ def test_literal_double_sum_on_tiny_inputs():
     assert np.max(np.abs(got - want)) <= 1e-13 * np.abs(want).max()
 
 
+def test_hand_solved_two_by_two():
+    """nao = n_mo = 2, B = [[1, 2], [3, 4]] (unsymmetric), C = [[1, 2], [3, 5]]: C^T B C by hand.
+    B C = [[7, 12], [15, 26]];  C^T (B C) = [[1*7 + 3*15, 1*12 + 3*26], [2*7 + 5*15, 2*12 + 5*26]] = [[52, 90], [89, 154]]."""
+    B = np.array([[[1.0, 2.0], [3.0, 4.0]]])
+    C = np.array([[1.0, 2.0], [3.0, 5.0]])
+    assert np.array_equal(oracle.ao_to_mo(B, C), np.array([[[52.0, 90.0], [89.0, 154.0]]]))
+
+
+def test_agrees_with_library_matmul():
+    """C^T B C through numpy's matmul (a library routine the oracle does not call) on a non-square C."""
+    rng = np.random.default_rng(5)
+    B, C = _case(rng, 4, 11, 7, sym=False)
+    want = np.matmul(C.T[None], np.matmul(B, C[None]))
+    assert np.max(np.abs(oracle.ao_to_mo(B, C) - want)) <= 1e-13 * np.abs(want).max()
+
+
 def test_identity_permutation_and_selection():
     rng = np.random.default_rng(2)
     B, _ = _case(rng, 4, 6, 6)

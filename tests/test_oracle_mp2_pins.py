@@ -127,3 +127,22 @@ def test_one_auxiliary_function_sox_is_minus_half_the_direct_term():
     d = oracle.mp2_direct(B, eps, occ, 0.01, o)
     sox = oracle.mp2(B, eps, occ, 0.01, o, sox_only=True)
     assert np.max(np.abs(sox + 0.5 * d)) <= 1e-13 * np.abs(d).max()
+
+
+@pytest.mark.parametrize("sym,sox_only", [(True, False), (False, False), (False, True)])
+def test_states_restriction_equals_the_full_call(sym, sox_only):
+    """oracle.mp2(states=S) (the gathered-copy variant used at sizes where the full sum is unaffordable) is the S x S
+    block of the full literal call, for unsorted S with B NOT symmetric (so a row gather taken for a column gather, or
+    (p S|ai) read as (S p|ai), shows), and for the exchange part alone."""
+    rng = np.random.default_rng(11)
+    N, o, naux = 9, 4, 5
+    B, eps, occ = _case(rng, N, o, naux, sym=sym)
+    full = oracle.mp2(B, eps, occ, 0.05, o, sox_only=sox_only)
+    S = [7, 0, 3, 4]
+    part = oracle.mp2(B, eps, occ, 0.05, o, sox_only=sox_only, states=S)
+    assert part.shape == (4, 4)
+    assert np.max(np.abs(part - full[np.ix_(S, S)])) <= 1e-13 * np.abs(full).max()
+    one = oracle.mp2(B, eps, occ, 0.05, o, sox_only=sox_only, states=[5])
+    assert one[0, 0] == pytest.approx(full[5, 5], rel=1e-12)
+    allS = oracle.mp2(B, eps, occ, 0.05, o, sox_only=sox_only, states=list(range(N)))
+    assert np.max(np.abs(allS - full)) <= 1e-13 * np.abs(full).max()
