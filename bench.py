@@ -1,21 +1,28 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the qsGW Sigma^c build on B200.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload large|xl|medium|small|tiny]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload xl|large|medium|small|tiny] [--shard replicas|poles]
   python bench.py --impl reference ...      # the CPU oracle timed on the host cores (bounded sample per step)
 
 A "step" is one pass of the whole hot path -- pack, stage 1, stage 2, stage 3 for every pole chunk, and
-the epilogue -- i.e. one Sigma^c build (qsgw_sigma_build through the C ABI) on seeded synthetic inputs of
-the named BASELINE.json config.  `value` = F_min / t in TFLOP/s (F_min = F1 + F2sym + F3,
-the least dense FP64 work the method needs, so the figure cannot be inflated by redundant work);
-`ms_per_step` = ms per build.  Inputs are resident in HBM for `value`; `e2e` repeats the build through
-qsgw_sigma_build_host with pinned HOST buffers, H2D/D2H copies inside the timed region.
-N > 1: the path does not shard in this scope ("replicas only"): every rank builds its own
-Sigma (seed + rank); the only collectives are the timing barrier and the max-over-ranks of the time.
+the epilogue -- i.e. one Sigma^c build through the C ABI on seeded synthetic inputs of the named BASELINE.json config.
+The default workload is `xl`, the largest single-GPU configuration (BASELINE.json's metric names no config); its Z
+(130 GB) is produced range by range on the device and fed through qsgw_sigma_begin / _add_poles / _finish.
+`value` = F_min / t in TFLOP/s (F_min = F1 + F2sym + F3, the least dense FP64 work the method needs,
+so the figure cannot be inflated by redundant work); `ms_per_step` = ms per build.  Inputs are resident in HBM for
+`value`; `e2e` repeats the build through qsgw_sigma_build_host with pinned HOST buffers, H2D/D2H copies inside the timed
+region.  Every number in the line is measured in this run (the FP64 roofline is cross-checked by an in-run probe); the
+one exception, `roofline.traffic`, is the DRAM byte count of a committed ncu capture and names the file it comes from.
+
+N > 1: `--shard replicas` (default): every rank builds its own Sigma (seed + rank), the only collectives
+are the timing barrier and the max-over-ranks of the time, "scaling": "weak".  `--shard poles`: ONE
+Sigma, rank r builds the pole slice qsgw_sigma_pole_slice gives it and one all-reduce of the N x N matrix finishes the
+build, "scaling": "strong".
 """
 from __future__ import annotations
 
 import argparse
+import ctypes
 import json
 import os
 import statistics
@@ -30,10 +37,16 @@ if ROOT not in sys.path:
 
 METRIC = "sigma_c_build_fp64_tflops"
 UNIT = "TFLOP/s"
-# FP64 pipe of sm_100a: DMMA.8x8x4 and DFMA both retire 64 FMA/clk/SM (measured: profiles/r01_fp64_peaks.md)
+# FP64 pipe of sm_100a: DMMA.8x8x4 and DFMA both retire 64 FMA/clk/SM (checked in every run by the probe below)
 FP64_FMA_PER_CLK_PER_SM = 64
-# dram__bytes_read.sum + dram__bytes_write.sum of one stage-2 launch over a full s-block (profiles/r01_full_large.md)
-NCU_STAGE2_DRAM_BYTES_PER_LAUNCH = {"large": 38.731918e9 + 11.789630e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE stage-2 launch over a full s-block, from committed `ncu --set full`
+# summaries (recorded numbers, not measurements of this run; the JSON line names the file)
+NCU_STAGE2_DRAM_BYTES_PER_LAUNCH = {}
+
+
+def pole_range(cfg) -> int:
+    """Poles per qsgw_sigma_add_poles call when Z is streamed: two s-blocks, so every call crosses a w-chunk boundary."""
+    return 2 * (cfg.s_block or 2048)
 
 
 def _peaks():
@@ -50,6 +63,43 @@ def fp64_peak_tflops(n_sms: int = 148):
     pk, src = _peaks()
     mhz = float(pk.get("sm_max_mhz", 1965.0))
     return n_sms * FP64_FMA_PER_CLK_PER_SM * 2 * mhz * 1e6 / 1e12, src, pk
+
+
+def measure_fp64_rates(torch, stream_ptr: int, with_dgemm: bool = True):
+    """In-run cross-check of the derived FP64 peak: the register-resident DMMA loop and the LDS-fed DMMA loop of
+    libqsgw_fp64_probe.so (a bench-only library; best of 3, ~10 ms each) and, as an outside reference that is never on
+    the product path, a cuBLAS DGEMM 8192^3 through torch.matmul."""
+    from paper_2210_17093_b200 import build
+    out = {}
+    try:
+        lib = ctypes.CDLL(build.build_probe())
+        lib.qsgw_fp64_probe.argtypes = [ctypes.c_int] * 4 + [ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+        for name, mode in (("dmma_microbench", 0), ("lds_fed_dmma_microbench", 3)):
+            best = 0.0
+            for _ in range(3):
+                tf = ctypes.c_double()
+                if lib.qsgw_fp64_probe(mode, 20000, 0, 1, ctypes.c_void_p(stream_ptr), ctypes.byref(tf), None) == 0:
+                    best = max(best, tf.value)
+            out[name] = best or None
+    except Exception as e:      # the probe is a cross-check, not a dependency of the measurement
+        out["probe_error"] = str(e)
+    if with_dgemm:
+        try:
+            a = torch.randn((8192, 8192), dtype=torch.float64, device="cuda")
+            b = torch.randn((8192, 8192), dtype=torch.float64, device="cuda")
+            c = a @ b
+            best = 0.0
+            for _ in range(3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); c = a @ b; e1.record(); torch.cuda.synchronize()
+                best = max(best, 2 * 8192.0 ** 3 / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+            out["cublas_dgemm_8192"] = best
+            del a, b, c
+            torch.cuda.empty_cache()
+        except Exception as e:
+            out["dgemm_error"] = str(e)
+    out["how"] = "measured in this run (best of 3 each); reference figures, the roofline denominator is `value`"
+    return out
 
 
 class ClockSampler:
@@ -118,19 +168,27 @@ def _sample_poles(cfg, target_s=20.0, gflops_guess=12.0):
     return max(4, min(cfg.n_pole, n))
 
 
+def _host_inputs_for_reference(cfg, n_sample):
+    """B, eps, occ, Omega and the first n_sample columns of Z as numpy arrays.  Drawn on the GPU when the box has one
+    (the CPU generator needs minutes for the 32 GB of xl's B); only the oracle runs in the timed steps either way."""
+    import torch
+    import qsgw_inputs as qi
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    B = qi.make_B(cfg, dev).cpu().numpy()
+    Z = qi.make_Z(cfg, 0, n_sample, device=dev).cpu().numpy()
+    return B, qi.make_eps(cfg).numpy(), qi.make_occ(cfg).numpy(), qi.make_omega(cfg).numpy(), Z
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the host cores; each step a bounded pole sample."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    import numpy as np  # noqa: F401
     import oracle
     import qsgw_inputs as qi
     cfg = qi.CONFIGS[args.workload]
     n_sample = args.ref_poles or _sample_poles(cfg, target_s=6.0)
-    B = qi.make_B(cfg).numpy()
-    eps, occ, Om = qi.make_eps(cfg).numpy(), qi.make_occ(cfg).numpy(), qi.make_omega(cfg).numpy()
-    Z = qi.make_Z(cfg, 0, n_sample).numpy()
+    B, eps, occ, Om, Z = _host_inputs_for_reference(cfg, n_sample)
     times = []
     for it in range(args.warmup + args.steps):
         dt, flops = _cpu_oracle_sample(cfg, B, eps, occ, Om, Z, n_sample)
@@ -154,8 +212,9 @@ def run_reference(args):
 
 
 def _config_dict(cfg, args, extra=None):
+    par = "single" if args.gpus <= 1 else ("pole-sharded" if getattr(args, "shard", "replicas") == "poles" else "replicas")
     d = {"workload": cfg.name, "n_mo": cfg.n_mo, "n_occ": cfg.n_occ, "n_aux": cfg.n_aux, "n_pole": cfg.n_pole,
-         "s_block": cfg.s_block, "eta": cfg.eta, "seed": cfg.seed, "parallelism": "replicas" if args.gpus > 1 else "single",
+         "s_block": cfg.s_block, "eta": cfg.eta, "seed": cfg.seed, "parallelism": par,
          "l2": "inputs larger than L2 (B + Z >> 126 MB); no explicit flush"}
     if extra:
         d.update(extra)
@@ -163,7 +222,7 @@ def _config_dict(cfg, args, extra=None):
 
 
 def max_over_ranks(ms: float, world: int, device="cpu") -> float:
-    """Replicas only: the one data-free collective of the bench -- the max over ranks of a rank-local time."""
+    """The one data-free collective of the bench: the max over ranks of a rank-local time."""
     if world <= 1:
         return float(ms)
     import torch
@@ -174,7 +233,8 @@ def max_over_ranks(ms: float, world: int, device="cpu") -> float:
 
 
 def whole_job_value(flops_per_rank: float, world: int, ms_per_step: float) -> float:
-    """Weak scaling: every rank builds its own Sigma, so the job's TFLOP/s is world x flops over the slowest rank's time."""
+    """Weak scaling (replicas): every rank builds its own Sigma, so the job's TFLOP/s is world x flops over the slowest
+    rank's time.  Pole-sharded runs pass world = 1 and the flops of the ONE Sigma all ranks build together."""
     return world * flops_per_rank / (ms_per_step * 1e-3) / 1e12
 
 
@@ -193,25 +253,31 @@ def run_gpu(args):
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+    sharded = args.shard == "poles" and world > 1
 
     base = qi.CONFIGS[args.workload]
-    cfg = qi.Config(base.name, base.n_mo, base.n_occ, base.n_aux, base.n_pole, base.s_block, base.eta, base.seed + rank)
-    streaming = args.stream_poles or (cfg.name == "xl")
+    # replicas: every rank its own problem (seed + rank); pole-sharded: ONE problem, the same B on every rank
+    cfg = base if sharded else qi.Config(base.name, base.n_mo, base.n_occ, base.n_aux, base.n_pole, base.s_block, base.eta,
+                                         base.seed + rank)
+    s_lo, n_local = pkg.qsgw_sigma_pole_slice(cfg.n_pole, world, rank) if sharded else (0, cfg.n_pole)
+    rng = pole_range(cfg)
+    # Z resident when this rank's columns fit beside B and the workspace (<= 48 GB), else produced range by range
+    streaming = args.stream_poles or (8.0 * cfg.n_ov * n_local > 48e9)
     fl = qi.flop_model(cfg)
     nsm = torch.cuda.get_device_properties(dev).multi_processor_count
     peak, peak_src, pk = fp64_peak_tflops(nsm)
+    rates = measure_fp64_rates(torch, torch.cuda.current_stream().cuda_stream) if rank == 0 else None
 
     # ---- inputs, resident in HBM before the timed region
     B = qi.make_B(cfg, dev)
     eps, occ, Om = qi.make_eps(cfg).to(dev), qi.make_occ(cfg).to(dev), qi.make_omega(cfg).to(dev)
-    rng = cfg.s_block or 2048
     if streaming:
         Zbuf = [torch.empty((cfg.n_ov, rng), dtype=torch.float64, device=dev) for _ in range(2)]
         Z = None
         plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, rng, cfg.s_block)
     else:
-        Z = qi.make_Z(cfg, device=dev)
-        plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, cfg.s_block)
+        Z = qi.make_Z(cfg, s_lo, s_lo + n_local, device=dev)
+        plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, max(n_local, 1), cfg.s_block)
     pkg.qsgw_sigma_set_profiling(plan, True)
     Sigma = torch.empty((cfg.n_mo, cfg.n_mo), dtype=torch.float64, device=dev)
 
@@ -220,27 +286,29 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    def timed(fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); fn(); e1.record()
+        return (e0, e1)
+
     def one_build():
-        """Returns device ms of this build (CUDA events on the launch stream)."""
-        if not streaming:
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta, Sigma)
-            e1.record()
-            return [(e0, e1)]
-        # xl: Z (130 GB) is produced range by range on the device just before each add_poles call;
-        # the generation is outside the event pairs, every kernel of the path is inside one.
-        evs = []
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(); pkg.qsgw_sigma_begin(plan, B, eps, occ, cfg.eta); e1.record(); evs.append((e0, e1))
-        for k, s0 in enumerate(range(0, cfg.n_pole, rng)):
-            s1 = min(cfg.n_pole, s0 + rng)
-            zb = Zbuf[k % 2][:, : s1 - s0]
-            qi.make_Z(cfg, s0, s1, device=dev, out=zb)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(); pkg.qsgw_sigma_add_poles(plan, Om[s0:s1], zb); e1.record(); evs.append((e0, e1))
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(); pkg.qsgw_sigma_finish(plan, Sigma); e1.record(); evs.append((e0, e1))
+        """One Sigma^c build; returns the CUDA event pairs (on the launch stream) that bracket every kernel of the path."""
+        if not streaming and not sharded:
+            return [timed(lambda: pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta, Sigma))]
+        evs = [timed(lambda: pkg.qsgw_sigma_begin(plan, B, eps, occ, cfg.eta))]
+        if streaming:
+            # Z (130 GB at xl) is produced range by range on the device just before each add_poles call;
+            # the generation is outside the event pairs, every kernel of the path is inside one.
+            for k, s0 in enumerate(range(s_lo, s_lo + n_local, rng)):
+                s1 = min(s_lo + n_local, s0 + rng)
+                zb = Zbuf[k % 2][:, : s1 - s0]
+                qi.make_Z(cfg, s0, s1, device=dev, out=zb)
+                evs.append(timed(lambda: pkg.qsgw_sigma_add_poles(plan, Om[s0:s1], zb)))
+        elif n_local > 0:
+            evs.append(timed(lambda: pkg.qsgw_sigma_add_poles(plan, Om[s_lo:s_lo + n_local], Z)))
+        evs.append(timed(lambda: pkg.qsgw_sigma_finish(plan, Sigma)))
+        if sharded:   # the exchange step of the sharded path: one all-reduce of the N x N matrix, inside the timed region
+            evs.append(timed(lambda: pkg.allreduce_sigma(Sigma)))
         return evs
 
     for _ in range(args.warmup):
@@ -256,87 +324,68 @@ def run_gpu(args):
         barrier()
         t_wall = time.perf_counter() - t_wall0
     step_ms = [sum(a.elapsed_time(b) for a, b in evs) for evs in all_events]
-    total_ms = sum(step_ms)
-    total_ms = max_over_ranks(total_ms, world, dev)
+    total_ms = max_over_ranks(sum(step_ms), world, dev)
     stats = pkg.qsgw_sigma_get_stats(plan, reset=True)
     ms_per_step = total_ms / args.steps
-    value = whole_job_value(fl["F_min"], world, ms_per_step)
+    value = whole_job_value(fl["F_min"], 1 if sharded else world, ms_per_step)
     assert torch.isfinite(Sigma).all()
 
     out = None
     if rank == 0:
-        # dominant kernel: the stage-2 DMMA GEMM (w producer), 57 % of F_min
+        # dominant kernel: the stage-2 DMMA GEMM (w producer), 57 % of F_min; its launches and flops on THIS rank
         n2 = max(1, stats["launches_stage2"])
         s2_ms = stats["ms_stage2"] / n2
-        flops_per_launch = fl["F2sym"] * args.steps / n2
+        fl_local = qi.flop_model(cfg, n_local)
+        flops_per_launch = fl_local["F2sym"] * args.steps / n2
         achieved = flops_per_launch / (s2_ms * 1e-3) / 1e12
-        bf16_ratio_peak = float(pk.get("bf16_tflops", 1590.0)) * 45.0 / 2250.0
+        traffic = NCU_STAGE2_DRAM_BYTES_PER_LAUNCH.get(cfg.name)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "ms_per_build": ms_per_step, "ms_per_build_best": min(step_ms),
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": _config_dict(cfg, args, extra={"z_resident": not streaming, "flops_F_min": fl["F_min"], "flops_F_full": fl["F_full"]}),
-            "tflops_model_full": world * fl["F_full"] / (ms_per_step * 1e-3) / 1e12,
+            "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": _config_dict(cfg, args, extra={"z_resident": not streaming, "poles_per_add_poles_call": rng if streaming else n_local,
+                                                     "flops_F_min": fl["F_min"], "flops_F_full": fl["F_full"]}),
+            "tflops_model_full": (1 if sharded else world) * fl["F_full"] / (ms_per_step * 1e-3) / 1e12,
             "frac_of_fp64_peak": value / (world * peak),
             "fp64_peak_tflops": {"value": peak, "how": f"{nsm} SMs x {FP64_FMA_PER_CLK_PER_SM} FMA/clk x 2 x sm_max_mhz of MEASURED_PEAKS.json ({peak_src})",
-                                 "dmma_microbench": 36.74, "lds_fed_dmma_microbench": 37.01, "cublas_dgemm_8192": 35.44,
-                                 "source": "profiles/r01_fp64_peaks.md",
-                                 "bf16_measured_x_nominal_ratio": bf16_ratio_peak},
+                                 "in_run_checks": rates},
             "stage_ms_per_build": {k[3:]: stats[k] / args.steps for k in ("ms_pack", "ms_stage1", "ms_stage2", "ms_stage3", "ms_epilogue")},
-            "stage_tflops": {"stage1": fl["F1"] * args.steps / max(stats["ms_stage1"], 1e-9) / 1e9,
-                             "stage2": fl["F2sym"] * args.steps / max(stats["ms_stage2"], 1e-9) / 1e9,
-                             "stage3": fl["F3"] * args.steps / max(stats["ms_stage3"], 1e-9) / 1e9},
+            "stage_tflops": {"stage1": fl_local["F1"] * args.steps / max(stats["ms_stage1"], 1e-9) / 1e9,
+                             "stage2": fl_local["F2sym"] * args.steps / max(stats["ms_stage2"], 1e-9) / 1e9,
+                             "stage3": fl_local["F3"] * args.steps / max(stats["ms_stage3"], 1e-9) / 1e9},
             "roofline": {"bound": "tensor", "kernel": "gemm_tn_dmma_kernel<2,2,EpiPairScatter> (stage 2, w producer)",
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "launches": stats["launches_stage2"], "avg_launch_ms": s2_ms,
-                         "traffic": NCU_STAGE2_DRAM_BYTES_PER_LAUNCH.get(cfg.name), "traffic_unit": "bytes per launch (dram read + write, ncu --set full, profiles/r01_full_large.md)",
-                         "peak_source": f"FP64 pipe rate at max SM clock ({peak_src} MEASURED_PEAKS.json sm_max_mhz); no FP64 entry is measured there"},
+                         "traffic": traffic[0] if traffic else None,
+                         "traffic_source": (f"recorded: dram read + write bytes of one launch over a full s-block, ncu --set full, {traffic[1]}"
+                                            if traffic else "no committed ncu capture for this workload"),
+                         "peak_source": f"FP64 pipe rate at max SM clock ({peak_src} MEASURED_PEAKS.json sm_max_mhz; no FP64 entry is "
+                                        "measured there); cross-checked in this run, see fp64_peak_tflops.in_run_checks"},
             "gpu_launches": stats["kernel_launches"],
             "wall_s_timed_region": t_wall,
             "clocks": clocks.summary(),
         }
 
     # ---- e2e: the same build through the host-buffer entry point (rank-local, max over ranks)
-    e2e = None
-    if not args.no_e2e and not streaming:
-        hB, hZ = B.cpu().pin_memory(), Z.cpu().pin_memory()
-        hE, hO, hOm = eps.cpu().pin_memory(), occ.cpu().pin_memory(), Om.cpu().pin_memory()
-        hS = torch.empty((cfg.n_mo, cfg.n_mo), dtype=torch.float64).pin_memory()
-        del Z
-        torch.cuda.empty_cache()
-        for _ in range(args.e2e_warmup):
-            pkg.qsgw_sigma_build_host(plan, hB, hE, hO, hOm, hZ, cfg.eta, hS)
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(args.e2e_steps):
-            pkg.qsgw_sigma_build_host(plan, hB, hE, hO, hOm, hZ, cfg.eta, hS)
-        e1.record()
-        barrier()
-        ms = e0.elapsed_time(e1)
-        ms = max_over_ranks(ms, world, dev) / args.e2e_steps
-        h2d = sum(t.numel() * 8 for t in (hB, hE, hO, hOm, hZ))
-        e2e = {"value": whole_job_value(fl["F_min"], world, ms), "unit": UNIT, "ms_per_build": ms, "steps": args.e2e_steps,
-               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": hS.numel() * 8,
-               "how": "qsgw_sigma_build_host from pinned host tensors; uploads overlap the kernels range by range"}
-        assert torch.isfinite(hS).all()
-    elif rank == 0:
+    held = {"B": B, "Z": Z}          # handed over so that the device copies can be freed as soon as the host has them
+    del B, Z
+    if streaming:
+        del Zbuf
+    if args.no_e2e or sharded:
         e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
-               "how": "skipped (--no-e2e, or Z is produced range by range on the device for this workload)"}
+               "how": "skipped (--no-e2e, or pole-sharded run)"}
+        hB = hZ = None
+    else:
+        e2e, hB, hZ = _run_e2e(args, torch, pkg, qi, cfg, plan, held, eps, occ, Om, dev, world, fl, barrier)
+    held.clear()
+    torch.cuda.empty_cache()
 
     # ---- cpu_baseline: the oracle as it stands, on rank 0's host cores, bounded sample of the same workload
     if rank == 0:
         out["e2e"] = e2e
         if world == 1 and not args.no_cpu_baseline:
-            import oracle
-            n_sample = args.ref_poles or _sample_poles(cfg)
-            Zs = (hZ[:, :n_sample] if (e2e and e2e.get("value")) else qi.make_Z(cfg, 0, n_sample, device=dev).cpu()).numpy()
-            dt, flops = _cpu_oracle_sample(cfg, B.cpu().numpy(), eps.cpu().numpy(), occ.cpu().numpy(), Om.cpu().numpy(), Zs, n_sample)
-            out["cpu_baseline"] = {
-                "value": flops / dt / 1e12, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                "sample": f"{n_sample} of {cfg.n_pole} poles of '{cfg.name}', all {cfg.n_mo} states, full B ({dt:.1f} s); "
-                          f"whole build extrapolated linearly in poles: {dt * cfg.n_pole / n_sample:.0f} s",
-                "ms_per_build_extrapolated": dt * 1e3 * cfg.n_pole / n_sample}
+            out["cpu_baseline"] = _cpu_baseline(args, torch, qi, cfg, hB, hZ, eps, occ, Om, dev)
         else:
             out["cpu_baseline"] = None
         print(json.dumps(out), flush=True)
@@ -346,12 +395,94 @@ def run_gpu(args):
     return 0
 
 
+def _pinned_empty(torch, shape):
+    """A host tensor of exactly this size, page-locked in place (torch's pinned allocator rounds big requests up to a
+    power of two: 130 GB would become 256 GB)."""
+    t = torch.empty(shape, dtype=torch.float64)
+    rc = torch.cuda.cudart().cudaHostRegister(t.data_ptr(), t.numel() * 8, 0)
+    if int(rc) != 0:
+        raise RuntimeError(f"cudaHostRegister failed with {rc}")
+    return t
+
+
+def _unpin(torch, t):
+    if t is not None:
+        torch.cuda.cudart().cudaHostUnregister(t.data_ptr())
+
+
+def _run_e2e(args, torch, pkg, qi, cfg, plan, held, eps, occ, Om, dev, world, fl, barrier):
+    """The build through qsgw_sigma_build_host: B, eps, occ, Omega, Z in page-locked HOST memory, Sigma back to the host,
+    all copies inside the timed region.  Returns (e2e dict, host B, host Z) -- the host arrays also serve cpu_baseline."""
+    import psutil
+    need = 8.0 * (cfg.n_aux * cfg.n_mo ** 2 + cfg.n_ov * cfg.n_pole)
+    avail = psutil.virtual_memory().available
+    if need + 20e9 > avail:
+        return ({"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                 "how": f"skipped: the host copy of B and Z needs {need / 1e9:.0f} GB of page-locked memory, {avail / 1e9:.0f} GB available"},
+                None, None)
+    hB = _pinned_empty(torch, (cfg.n_aux, cfg.n_mo, cfg.n_mo))
+    hB.copy_(held.pop("B"))
+    hZ = _pinned_empty(torch, (cfg.n_ov, cfg.n_pole))
+    Z = held.pop("Z")
+    if Z is not None:
+        hZ.copy_(Z)
+        del Z
+    else:       # xl: Z never exists whole on the device; draw it range by range and move it to the host once, untimed
+        step = pole_range(cfg)
+        zb = torch.empty((cfg.n_ov, step), dtype=torch.float64, device=dev)
+        for s0 in range(0, cfg.n_pole, step):
+            s1 = min(cfg.n_pole, s0 + step)
+            qi.make_Z(cfg, s0, s1, device=dev, out=zb[:, : s1 - s0])
+            hZ[:, s0:s1].copy_(zb[:, : s1 - s0])
+        del zb
+    hE, hO, hOm = eps.cpu().pin_memory(), occ.cpu().pin_memory(), Om.cpu().pin_memory()
+    hS = torch.empty((cfg.n_mo, cfg.n_mo), dtype=torch.float64).pin_memory()
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    for _ in range(args.e2e_warmup):
+        pkg.qsgw_sigma_build_host(plan, hB, hE, hO, hOm, hZ, cfg.eta, hS)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.e2e_steps):
+        pkg.qsgw_sigma_build_host(plan, hB, hE, hO, hOm, hZ, cfg.eta, hS)
+    e1.record()
+    barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1), world, dev) / args.e2e_steps
+    h2d = sum(t.numel() * 8 for t in (hB, hE, hO, hOm, hZ))
+    assert torch.isfinite(hS).all()
+    return ({"value": whole_job_value(fl["F_min"], world, ms), "unit": UNIT, "ms_per_build": ms, "steps": args.e2e_steps,
+             "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": hS.numel() * 8,
+             "how": "qsgw_sigma_build_host from page-locked host tensors; uploads overlap the kernels"}, hB, hZ)
+
+
+def _cpu_baseline(args, torch, qi, cfg, hB, hZ, eps, occ, Om, dev):
+    import oracle
+    n_sample = args.ref_poles or _sample_poles(cfg)
+    if hB is None:
+        hB = qi.make_B(cfg, dev).cpu()
+        torch.cuda.empty_cache()
+    Zs = (hZ[:, :n_sample] if hZ is not None else qi.make_Z(cfg, 0, n_sample, device=dev).cpu()).numpy()
+    Bn, en, on, omn = hB.numpy(), eps.cpu().numpy(), occ.cpu().numpy(), Om.cpu().numpy()
+    dt, flops = _cpu_oracle_sample(cfg, Bn, en, on, omn, Zs, n_sample)
+    cores = oracle.num_threads()
+    res = {"value": flops / dt / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"{n_sample} of {cfg.n_pole} poles of '{cfg.name}', all {cfg.n_mo} states, full B ({dt:.1f} s); "
+                     f"whole build extrapolated linearly in poles: {dt * cfg.n_pole / n_sample:.0f} s",
+           "ms_per_build_extrapolated": dt * 1e3 * cfg.n_pole / n_sample}
+    if cfg.name in ("tiny", "small"):       # SURVEY.md 8(d): a one-core figure for the two smallest configs
+        oracle.set_num_threads(1)
+        dt1, _ = _cpu_oracle_sample(cfg, Bn, en, on, omn, Zs, n_sample)
+        oracle.set_num_threads(cores)
+        res["one_thread"] = {"value": flops / dt1 / 1e12, "unit": UNIT, "cores": 1, "seconds": dt1}
+    return res
+
+
 def run_gpu_diag(args):
     """--path diag: the next row of the scope table, measured to the same bar -- one step is one
     qsgw_sigma_diag_build (pack, stage 1, stage 2 per s-block, the G0W0 diagonal kernel per s-block) for all N
     states on an n_omega-point grid.  value = 1e9 complex Lehmann terms evaluated per second,
     N^2 * n_s * n_omega / t; the kernel is bound by the FP64 ALU rate (8 FP64-pipe instructions per term)."""
-    import numpy as np
     import torch
     import qsgw_inputs as qi
     import paper_2210_17093_b200 as pkg
@@ -412,7 +543,7 @@ def run_gpu_diag(args):
                                     "loop reaches 80 % of it (profiles/r01_fp64_peaks.md); 8 FP64-pipe instructions per term"},
         "gpu_launches": stats["kernel_launches"], "clocks": clocks.summary(),
         "e2e": {"value": None, "unit": "Gterm/s", "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
-                "how": "no host-buffer entry point for this row yet"},
+                "how": "B and Z stay on the device between the qsGW build and the diagonal: no host-buffer entry point for this row"},
     }
     if not args.no_cpu_baseline:
         import oracle
@@ -475,15 +606,16 @@ def run_gpu_aomo(args):
                         "avg_launch_ms": ms / 2, "traffic": None, "peak_source": f"FP64 pipe rate at max SM clock ({peak_src})"},
            "gpu_launches": 2 * args.steps, "clocks": clocks.summary(),
            "e2e": {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
-                   "how": "B stays on the device between the transform and the Sigma build"}}
+                   "how": "B stays on the device between the transform and the Sigma build: no host-buffer entry point for this row"}}
     if not args.no_cpu_baseline:
         import oracle
-        n_s = min(cfg.n_aux, 64)
+        n_s = max(1, min(cfg.n_aux, int(4e11 / (2.0 * float(cfg.n_mo) ** 4))))     # the oracle is the O(N^4) double sum per P
         t0 = time.perf_counter()
         oracle.ao_to_mo(B_ao[:n_s].cpu().numpy(), C.cpu().numpy())
         dt = time.perf_counter() - t0
-        out["cpu_baseline"] = {"value": 4.0 * float(cfg.n_mo) ** 3 * n_s / dt / 1e12, "unit": UNIT, "cores": os.cpu_count(),
-                               "kind": "oracle", "sample": f"{n_s} of {cfg.n_aux} auxiliary functions of '{cfg.name}' ({dt:.2f} s; numpy matmul)"}
+        out["cpu_baseline"] = {"value": 4.0 * float(cfg.n_mo) ** 3 * n_s / dt / 1e12, "unit": UNIT + " (GPU flop model / oracle time)",
+                               "cores": oracle.num_threads(), "kind": "oracle",
+                               "sample": f"{n_s} of {cfg.n_aux} auxiliary functions of '{cfg.name}' ({dt:.2f} s; the literal double sum, 2 N^4 flops per P)"}
     print(json.dumps(out), flush=True)
     return 0
 
@@ -540,14 +672,17 @@ def run_gpu_mp2(args):
                         "peak_source": f"FP64 pipe rate at max SM clock ({peak_src})"},
            "gpu_launches": stats["kernel_launches"], "clocks": clocks.summary(),
            "e2e": {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
-                   "how": "B, eps, occ stay on the device between the AO->MO transform and the build"}}
-    if not args.no_cpu_baseline and cfg.n_mo <= 120:
+                   "how": "B, eps, occ stay on the device between the AO->MO transform and the build: no host-buffer entry point for this row"}}
+    if not args.no_cpu_baseline:
         import oracle
+        states = [0, cfg.n_occ - 1, cfg.n_occ, cfg.n_mo - 1] if cfg.n_mo > 120 else None
         t0 = time.perf_counter()
-        oracle.mp2(B.cpu().numpy(), eps.cpu().numpy(), occ.cpu().numpy(), cfg.eta, cfg.n_occ)
+        oracle.mp2(B.cpu().numpy(), eps.cpu().numpy(), occ.cpu().numpy(), cfg.eta, cfg.n_occ, states=states)
         dt = time.perf_counter() - t0
-        out["cpu_baseline"] = {"value": (f_direct + f_sox) / dt / 1e12, "unit": UNIT + " (GPU flop model / oracle time)",
-                               "cores": oracle.num_threads(), "kind": "oracle", "sample": f"whole '{cfg.name}' build ({dt:.1f} s)"}
+        what = f"whole '{cfg.name}' build" if states is None else f"{len(states)} of {cfg.n_mo} output states of '{cfg.name}', all internal sums"
+        out["cpu_baseline"] = {"value": (f_direct + f_sox) * (1.0 if states is None else len(states) / N) / dt / 1e12,
+                               "unit": UNIT + " (GPU flop model, scaled by the share of output rows / oracle time)",
+                               "cores": oracle.num_threads(), "kind": "oracle", "sample": f"{what} ({dt:.1f} s)"}
     print(json.dumps(out), flush=True)
     pkg.qsgw_sigma_destroy(plan)
     return 0
@@ -556,11 +691,13 @@ def run_gpu_mp2(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="large", choices=["tiny", "small", "medium", "large", "xl"])
-    ap.add_argument("--stream-poles", action="store_true", help="produce Z range by range (always on for xl)")
+    ap.add_argument("--workload", default="xl", choices=["tiny", "small", "medium", "large", "xl"])
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "poles"],
+                    help="N > 1: independent replicas (weak scaling, the default) or ONE Sigma sharded over the poles + all-reduce")
+    ap.add_argument("--stream-poles", action="store_true", help="produce Z range by range (always on when Z does not fit)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--e2e-warmup", type=int, default=1)

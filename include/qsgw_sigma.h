@@ -193,6 +193,19 @@ int qsgw_ri_ao_to_mo(const double *B_ao, const double *C, int n_aux, int n_ao, i
                      void *cuda_stream);
 size_t qsgw_ri_ao_to_mo_work_doubles(int n_aux, int n_ao, int n_mo);
 
+/*
+ * Row 8(e) / 8(f).4 of the scope table: the build shards over the pole index s.  Sigma is a plain sum over s (Eq. (17),
+ * PAPER.md:149), V[:,s] depends only on Z[:,s] and w^s only on V[:,s], so rank r of n_ranks runs
+ * qsgw_sigma_begin / _add_poles / _finish on the contiguous slice Omega[s0 .. s0+n), Z[:, s0 .. s0+n) of the poles (B, eps,
+ * occ replicated) and ONE all-reduce(sum) of the n_mo x n_mo Sigma over the ranks finishes the build (the paper itself is
+ * single-GPU; multi-GPU is its future work).  This helper is the partition: slices are contiguous, disjoint,
+ * cover [0, n_pole), start at multiples of 32 poles (the k-tile depth of stage 3; keeps Z + s0 16-byte aligned) and differ
+ * by at most 32 poles in length.  A rank may get n = 0 (more ranks than 32-pole groups): it calls begin and finish only and
+ * contributes Sigma = 0.  Pure host arithmetic, no device needed.
+ * Errors: INVALID_ARG if n_pole < 1, n_ranks < 1, rank outside [0, n_ranks) or s0 / n is NULL.
+ */
+int qsgw_sigma_pole_slice(int64_t n_pole, int n_ranks, int rank, int64_t *s0, int64_t *n);
+
 /* Free the workspace and the plan.  Synchronises the plan's stream first.  NULL is accepted. */
 int qsgw_sigma_destroy(qsgw_sigma_plan *plan);
 

@@ -429,3 +429,13 @@ int qsgw_oracle_ao_to_mo(int naux, int nao, int nmo, const double *B_ao, const d
   }
   return 0;
 }
+
+/* Number of OpenMP threads the oracle uses from now on (n < 1: leave unchanged).  Not arithmetic: bench.py uses it to time
+ * the oracle on one host core next to the all-cores figure. */
+void qsgw_oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n >= 1) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}

@@ -41,6 +41,8 @@ def _load():
         ip = ctypes.POINTER(ctypes.c_int)
         i64 = ctypes.c_int64
         lib.qsgw_oracle_num_threads.restype = ctypes.c_int
+        lib.qsgw_oracle_set_num_threads.restype = None
+        lib.qsgw_oracle_set_num_threads.argtypes = [ctypes.c_int]
         lib.qsgw_oracle_D.restype = ctypes.c_double
         lib.qsgw_oracle_D.argtypes = [ctypes.c_double] * 5
         lib.qsgw_oracle_pole_weights.restype = None
@@ -80,6 +82,11 @@ def _f64(a, shape=None):
 def num_threads() -> int:
     """OpenMP threads the oracle will use (its `cores` figure when timed as the CPU baseline)."""
     return int(_load().qsgw_oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    """Use n OpenMP threads from now on (bench.py's one-core figure)."""
+    _load().qsgw_oracle_set_num_threads(int(n))
 
 
 def D(occ_m: float, eps_m: float, Omega_s: float, omega: float, eta: float) -> float:

@@ -29,6 +29,7 @@ EXPORTS = (
     "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
     "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_mp2_direct_build", "qsgw_mp2_build", "qsgw_ri_ao_to_mo", "qsgw_ri_ao_to_mo_work_doubles", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
     "qsgw_sigma_limit_pole_batch", "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_set_debug", "qsgw_sigma_version",
+    "qsgw_sigma_pole_slice",
 )
 
 
@@ -100,6 +101,8 @@ def load_library() -> ctypes.CDLL:
         lib.qsgw_sigma_set_profiling.argtypes = [vp, ci]
         lib.qsgw_sigma_get_stats.restype = ci
         lib.qsgw_sigma_get_stats.argtypes = [vp, ctypes.POINTER(qsgw_sigma_stats), ci]
+        lib.qsgw_sigma_pole_slice.restype = ci
+        lib.qsgw_sigma_pole_slice.argtypes = [i64, ci, ci, ctypes.POINTER(i64), ctypes.POINTER(i64)]
         lib.qsgw_sigma_set_debug.restype = ci
         lib.qsgw_sigma_set_debug.argtypes = [vp, ci]
         lib.qsgw_sigma_version.restype = ci
@@ -332,6 +335,13 @@ def qsgw_sigma_get_stats(plan: Plan, reset: bool = False) -> dict:
 def qsgw_sigma_set_debug(plan: Plan, on: bool) -> None:
     """Device-side precondition checks (B symmetric and finite, occ in [0,1], Omega > 0) in begin / add_poles."""
     _check(load_library().qsgw_sigma_set_debug(plan.handle, 1 if on else 0), plan.handle)
+
+
+def qsgw_sigma_pole_slice(n_pole: int, n_ranks: int, rank: int):
+    """(s0, n): the contiguous slice of the pole index that rank `rank` of `n_ranks` builds (pure host arithmetic)."""
+    s0, n = ctypes.c_int64(), ctypes.c_int64()
+    _check(load_library().qsgw_sigma_pole_slice(int(n_pole), int(n_ranks), int(rank), ctypes.byref(s0), ctypes.byref(n)), None)
+    return int(s0.value), int(n.value)
 
 
 def qsgw_sigma_version() -> int:

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libqsgw_sigma.so")
 TESTHOOKS_LIB_PATH = os.path.join(_HERE, "libqsgw_sigma_testhooks.so")
 PROBE_LIB_PATH = os.path.join(_HERE, "libqsgw_fp64_probe.so")
 SOURCES = ["qsgw_sigma.cu"]
-HEADERS = ["dmma_gemm.cuh", "sigma_kernels.cuh", os.path.join("..", "..", "include", "qsgw_sigma.h")]
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith(".cuh")) + [os.path.join("..", "..", "include", "qsgw_sigma.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "--shared", "-Xcompiler", "-fPIC", "-cudart", "shared",

@@ -19,6 +19,7 @@
 
 #include "../../include/qsgw_sigma.h"
 #include "sigma_kernels.cuh"
+#include "sigma_tma.cuh"
 
 using namespace qsgw;
 
@@ -46,6 +47,9 @@ struct qsgw_sigma_plan {
   // workspace
   int64_t n_pair = 0, ldp = 0, ld_aux = 0, ldv = 0, ldw = 0;
   int nsplit = 0, m_per_split = 0, ntile_1d = 0;
+  int tq = 0, ntq = 0;       // stage-3 tile width (q columns, a multiple of 8 chosen for n_mo) and tiles per row
+  bool legacy_stage3 = false;
+  int dbg_flags = 0;
   double *Bp = nullptr, *BovT = nullptr, *V = nullptr, *W = nullptr, *Tpart = nullptr, *mp2_omega = nullptr, *mp2_y = nullptr;
   int2 *pairs = nullptr;
   size_t bytes = 0;
@@ -167,7 +171,8 @@ cudaError_t configure_kernels_for_device(int dev) {
   set(allow_smem(gemm_tn_dmma_kernel<1, 2, EpiStore>, kGemmSmemBytes));
   set(allow_smem(gemm_tn_dmma_kernel<1, 1, EpiStore>, kGemmSmemBytes));
   set(allow_smem(gemm_tn_dmma_kernel<2, 2, EpiPairScatter>, kGemmSmemBytes));
-  set(allow_smem(sigma_accumulate_kernel, kSigmaSmemBytes));
+  set(allow_smem(sigma_accumulate_kernel, kSigmaSmemBudget + 1024));
+  set(allow_smem(sigma_accumulate_cpasync_kernel, kOldSigmaSmemBytes));
   set(allow_smem(sigma_diag_kernel, kDiagSmemMax));
   if (e == cudaSuccess && dev >= 0 && dev < kMaxDevices) g_attr_done[dev] = true;
   return e;
@@ -254,12 +259,62 @@ int run_stage2(qsgw_sigma_plan *p, const double *Vc, int sc, double alpha) {
   return launch_gemm<2>(p, p->Bp, p->ldp, Vc, p->ldv, (int)p->n_pair, sc, p->n_aux, epi);
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point lookup (no link-time dependency on libcuda)
+using EncodeTiledFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn tensor_map_encoder() {
+  static EncodeTiledFn fn = [] {
+    void *ptr = nullptr;
+    cudaDriverEntryPointQueryResult st;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &st) != cudaSuccess ||
+        st != cudaDriverEntryPointSuccess)
+      ptr = nullptr;
+    cudaGetLastError();
+    return reinterpret_cast<EncodeTiledFn>(ptr);
+  }();
+  return fn;
+}
+
+// 3-D tensor map of a stage-3 operand X[m][p][s] (row m*N + p, leading dimension ld, sc valid poles): box = 16 poles
+// (128 bytes, the swizzle span) x box_rows rows of one m; rows >= N and poles >= sc read as zeros.
+int encode_operand_map(qsgw_sigma_plan *p, CUtensorMap *map, const double *X, int64_t ld, int sc, int box_rows) {
+  EncodeTiledFn enc = tensor_map_encoder();
+  if (!enc) return fail(p, QSGW_SIGMA_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  const cuuint64_t dims[3] = {(cuuint64_t)sc, (cuuint64_t)p->n_mo, (cuuint64_t)p->n_mo};
+  const cuuint64_t strides[2] = {(cuuint64_t)ld * 8, (cuuint64_t)p->n_mo * (cuuint64_t)ld * 8};
+  const cuuint32_t box[3] = {16, (cuuint32_t)box_rows, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double *>(X), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    char buf[160];
+    snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed with %d (ld = %lld, sc = %d, rows = %d)", (int)r, (long long)ld, sc, box_rows);
+    return fail(p, QSGW_SIGMA_ERR_CUDA, buf);
+  }
+  return QSGW_SIGMA_OK;
+}
+
 // Stage 3 for one chunk: Tpart[z] += (WA.D) WB^T over the internal states of split z and the chunk's sc poles
 int run_stage3(qsgw_sigma_plan *p, const double *WA, int64_t ldA, const double *WB, int64_t ldB, const double *Omega_c, int sc) {
   ScopedTimer t(p, kStage3);
-  const int ntp = (p->n_mo + kTP - 1) / kTP, ntq = (p->n_mo + kTQ - 1) / kTQ;
-  sigma_accumulate_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kSigmaSmemBytes, p->stream>>>(
-      WA, ldA, WB, ldB, p->eps, p->occ, Omega_c, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart);
+  if (p->legacy_stage3) {
+    const int ntp = (p->n_mo + kOldTP - 1) / kOldTP, ntq = (p->n_mo + kOldTQ - 1) / kOldTQ;
+    sigma_accumulate_cpasync_kernel<<<dim3(ntp * ntq, p->nsplit), kThreads, kOldSigmaSmemBytes, p->stream>>>(
+        WA, ldA, WB, ldB, p->eps, p->occ, Omega_c, p->n_mo, sc, p->eta * p->eta, p->m_per_split, ntq, p->Tpart);
+  } else {
+    CUtensorMap mapA, mapB;
+    int rc;
+    if ((rc = encode_operand_map(p, &mapA, WA, ldA, sc, kTP))) return rc;
+    if ((rc = encode_operand_map(p, &mapB, WB, ldB, sc, p->tq))) return rc;
+    const SigmaRings rings = sigma_rings(p->tq);
+    const int ntp = (p->n_mo + kTP - 1) / kTP;
+    sigma_accumulate_kernel<<<dim3(ntp * p->ntq, p->nsplit), kThreads, rings.smem_bytes, p->stream>>>(
+        mapA, mapB, p->eps, p->occ, Omega_c, p->n_mo, sc, p->eta * p->eta, p->m_per_split, p->ntq, p->tq, rings.nA, rings.nB,
+        p->Tpart, p->dbg_flags);
+  }
   p->kernel_launches += 1;
   QSGW_CUDA(p, cudaGetLastError());
   return QSGW_SIGMA_OK;
@@ -542,7 +597,17 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
   p->v_cols_alloc = p->v_cols;
   p->ldw = round_up(p->s_chunk, 2);
   // split-K of stage 3 over the internal state m: enough CTAs for ~40 waves of the SMs (ragged edge tiles run 2-3x shorter than full ones: the tail of a launch is one CTA long), at most N splits
-  const int nt2 = ((n_mo + kTP - 1) / kTP) * ((n_mo + kTQ - 1) / kTQ);
+  // stage-3 tile width: the fewest tiles of at most 256 columns, all (but rounding) equally wide, so that no CTA is
+  // left with a sliver of columns that amortises the D evaluations of its p rows badly
+  p->ntq = (n_mo + kTQMax - 1) / kTQMax;
+  p->tq = std::min<int>(kTQMax, (int)round_up((n_mo + p->ntq - 1) / p->ntq, 16));   // a multiple of 16 columns: the four sub-partitions' DMMA warps get equal shares
+  {
+    const char *legacy = std::getenv("QSGW_SIGMA_STAGE3_LEGACY");
+    p->legacy_stage3 = legacy && legacy[0] == '1';
+    const char *df = std::getenv("QSGW_SIGMA_DBG");
+    p->dbg_flags = df ? atoi(df) : 0;
+  }
+  const int nt2 = ((n_mo + kTP - 1) / kTP) * (p->legacy_stage3 ? (n_mo + kOldTQ - 1) / kOldTQ : p->ntq);
   int want = (40 * prop.multiProcessorCount + nt2 - 1) / nt2;
   want = std::max(1, std::min(want, n_mo));
   p->m_per_split = (n_mo + want - 1) / want;
@@ -750,6 +815,17 @@ int qsgw_ri_ao_to_mo(const double *B_ao, const double *C, int n_aux, int n_ao, i
                 : launch_gemm_on<2, 1>(nullptr, stream, sms, work, ldt, C, n_mo, n_mo, n_mo, n_ao, epi, n_aux, sT, 0);
     if (rc) return rc;
   }
+  return QSGW_SIGMA_OK;
+}
+
+int qsgw_sigma_pole_slice(int64_t n_pole, int n_ranks, int rank, int64_t *s0, int64_t *n) {
+  if (n_pole < 1 || n_ranks < 1 || rank < 0 || rank >= n_ranks || !s0 || !n)
+    return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "pole_slice: need n_pole >= 1, 0 <= rank < n_ranks, non-NULL outputs");
+  constexpr int64_t kGranule = 32;
+  const int64_t units = (n_pole + kGranule - 1) / kGranule;
+  const int64_t lo = units * rank / n_ranks, hi = units * (rank + 1) / n_ranks;   // units <= 2^58: no overflow for n_ranks < 32
+  *s0 = std::min(n_pole, lo * kGranule);
+  *n = std::min(n_pole, hi * kGranule) - *s0;
   return QSGW_SIGMA_OK;
 }
 

@@ -115,7 +115,7 @@ __global__ void check_range_kernel(const double *__restrict__ x, int64_t n, doub
 // x/(x^2+eta^2) without the IEEE division's slow path: y = x^2+eta^2, r = MUFU.RCP64H(y) (relative error
 // e = 1 - y r, |e| <= 2^-20 measured), 1/y = r (1 + e + e^2 + O(e^3)), so x/y = q + q (e + e^2) with q = x r:
 // 5 FP64-pipe instructions, error <= 1 ulp (|e|^3 = 2^-60).  y >= eta^2 > 0 is never subnormal for physical energies.
-__device__ __forceinline__ double lehmann_term(double x, double eta2) {
+__device__ __forceinline__ double lehmann_term_old(double x, double eta2) {
   const double y = fma(x, x, eta2);
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
@@ -128,9 +128,9 @@ __device__ __forceinline__ double lehmann_term(double x, double eta2) {
 // OCC: 1 = f_m == 1 (occupied), 0 = f_m == 0 (virtual), 2 = fractional (both terms)
 template <int OCC>
 __device__ __forceinline__ double denominator_D(double d, double Omega_s, double occ_m, double eta2) {
-  if (OCC == 1) return lehmann_term(d + Omega_s, eta2);
-  if (OCC == 0) return lehmann_term(d - Omega_s, eta2);
-  return occ_m * lehmann_term(d + Omega_s, eta2) + (1.0 - occ_m) * lehmann_term(d - Omega_s, eta2);
+  if (OCC == 1) return lehmann_term_old(d + Omega_s, eta2);
+  if (OCC == 0) return lehmann_term_old(d - Omega_s, eta2);
+  return occ_m * lehmann_term_old(d + Omega_s, eta2) + (1.0 - occ_m) * lehmann_term_old(d - Omega_s, eta2);
 }
 
 // Stage-3 CTA tile: 64 p rows x 256 q columns, k-tiles of 16 poles at one internal state m.  The tile is wide
@@ -138,23 +138,23 @@ __device__ __forceinline__ double denominator_D(double d, double Omega_s, double
 // 64 x 16 evaluations against 64 x 256 x 16 FMA.  The 8 consumer warps are laid out 2 (p) x 4 (q), each owning
 // 4 x 8 DMMA fragments interleaved across the tile (p rows 16i + 8wmi + g, q columns 32j + 8wni + g), so ragged
 // edge tiles shed whole fragments evenly: granule 16 rows x 32 columns.
-constexpr int kTP = 64;
-constexpr int kTQ = 256;
+constexpr int kOldTP = 64;
+constexpr int kOldTQ = 256;
 constexpr int kSigmaStages = 5;
-constexpr int kSigmaStageDoubles = (kTP + kTQ) * kBK;   // unpadded [row][16] tiles, XOR-swizzled (see sw_col)
-constexpr size_t kSigmaSmemBytes = (size_t)kSigmaStages * kSigmaStageDoubles * sizeof(double) + 2 * kSigmaStages * sizeof(uint64_t);
+constexpr int kSigmaStageDoubles = (kOldTP + kOldTQ) * kBK;   // unpadded [row][16] tiles, XOR-swizzled (see sw_col)
+constexpr size_t kOldSigmaSmemBytes = (size_t)kSigmaStages * kSigmaStageDoubles * sizeof(double) + 2 * kSigmaStages * sizeof(uint64_t);
 
 // Shared tiles of stage 3 are [row][16] doubles with the column index XOR-swizzled by 4 * (row & 3): a DMMA fragment
 // load (lanes g = 0..7 rows, t = 0..3 columns 4kk + t) then hits 16 distinct 8-byte bank pairs per half warp, and a
 // 16-byte cp.async chunk (2 columns) stays contiguous.  No padding: 5 stages of (64 + 256) x 16 doubles fit.
 __device__ __forceinline__ int sw_col(int row, int col) { return col ^ ((row & 3) << 2); }
 
-struct SigmaFragMap {
+struct OldSigmaFragMap {
   int wmi, wni, g, t;
   int mi_cnt, nj_cnt;   // fragments of this warp with at least one valid row / column (warp-uniform)
-  __device__ __forceinline__ SigmaFragMap(int warp, int lane, int rows_valid, int cols_valid) {
+  __device__ __forceinline__ OldSigmaFragMap(int warp, int lane, int rows_valid, int cols_valid) {
     wmi = warp & 1; wni = warp >> 1; g = lane >> 2; t = lane & 3;
-    const int rb = min(kTP / 8, (max(rows_valid, 0) + 7) >> 3), cb = min(kTQ / 8, (max(cols_valid, 0) + 7) >> 3);
+    const int rb = min(kOldTP / 8, (max(rows_valid, 0) + 7) >> 3), cb = min(kOldTQ / 8, (max(cols_valid, 0) + 7) >> 3);
     mi_cnt = max(0, (rb - wmi + 1) >> 1);
     nj_cnt = max(0, (cb - wni + 3) >> 2);
   }
@@ -221,16 +221,16 @@ __device__ __forceinline__ void mma_ktile_sigma_ragged(double (&acc)[4][8][2], c
 // ahead; each producer thread then multiplies the chunks of the p rows it copied itself by D(m, s, eps_p) in
 // place: the scaled operand A = w.D exists only in shared memory.  The 8 consumer warps run LDS + DMMA only.
 __global__ void __launch_bounds__(kThreads, 1)
-sigma_accumulate_kernel(const double *__restrict__ WA, int64_t ldA, const double *__restrict__ WB, int64_t ldB,
+sigma_accumulate_cpasync_kernel(const double *__restrict__ WA, int64_t ldA, const double *__restrict__ WB, int64_t ldB,
                         const double *__restrict__ eps, const double *__restrict__ occ, const double *__restrict__ Omega,
                         int n_mo, int s_c, double eta2, int m_per_split, int ntq, double *__restrict__ Tpart) {
   extern __shared__ __align__(16) double smem[];
-  // stage st: p rows at smem + st*kSigmaStageDoubles (already scaled by D when released), q rows kTP*kBK further
+  // stage st: p rows at smem + st*kSigmaStageDoubles (already scaled by D when released), q rows kOldTP*kBK further
   uint64_t *full = reinterpret_cast<uint64_t *>(smem + kSigmaStages * kSigmaStageDoubles);
   uint64_t *empty = full + kSigmaStages;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int tp = blockIdx.x / ntq, tq = blockIdx.x - tp * ntq;
-  const int p0 = tp * kTP, q0 = tq * kTQ;
+  const int p0 = tp * kOldTP, q0 = tq * kOldTQ;
   const int m_begin = blockIdx.y * m_per_split;
   const int m_end = min(n_mo, m_begin + m_per_split);
   const int KTS = (s_c + kBK - 1) / kBK;         // k-tiles per m
@@ -251,14 +251,14 @@ sigma_accumulate_kernel(const double *__restrict__ WA, int64_t ldA, const double
     const int pt = tid - kConsumerThreads, pw = pt >> 5;
     const int c2 = (lane & 7) * 2;                // this thread's two columns of every k-tile
     const int rsub = lane >> 3;                   // rows rA0 + 4j (j < 4) of the p tile, rB0 + 4j (j < 16) of the q tile
-    const int rA0 = pw * (kTP / 4) + rsub, rB0 = pw * (kTQ / 4) + rsub;
-    const int nrowA = max(0, min(kTP / 16, (n_mo - p0 - rA0 + 3) >> 2));   // valid rows among its 4 / 16
-    const int nrowB = max(0, min(kTQ / 16, (n_mo - q0 - rB0 + 3) >> 2));
+    const int rA0 = pw * (kOldTP / 4) + rsub, rB0 = pw * (kOldTQ / 4) + rsub;
+    const int nrowA = max(0, min(kOldTP / 16, (n_mo - p0 - rA0 + 3) >> 2));   // valid rows among its 4 / 16
+    const int nrowB = max(0, min(kOldTQ / 16, (n_mo - q0 - rB0 + 3) >> 2));
     // all of a thread's rows are congruent to rsub mod 4, so one swizzled column offset serves them all
     const int csw = sw_col(rsub, c2);
-    double eps_p[kTP / 16];
+    double eps_p[kOldTP / 16];
 #pragma unroll
-    for (int j = 0; j < kTP / 16; ++j) eps_p[j] = (j < nrowA) ? __ldg(eps + p0 + rA0 + 4 * j) : 0.0;
+    for (int j = 0; j < kOldTP / 16; ++j) eps_p[j] = (j < nrowA) ? __ldg(eps + p0 + rA0 + 4 * j) : 0.0;
     const int64_t stepA = 4 * ldA, stepB = 4 * ldB;
     constexpr int kAhead = 2;                     // k-tiles whose cp.async are in flight ahead of the scaling
 
@@ -274,14 +274,14 @@ sigma_accumulate_kernel(const double *__restrict__ WA, int64_t ldA, const double
         const double *srcA = WA + ((int64_t)ld_m * n_mo + p0 + rA0) * ldA + s;
         const double *srcB = WB + ((int64_t)ld_m * n_mo + q0 + rB0) * ldB + s;
         double *dstA = smem + ld_st * kSigmaStageDoubles + rA0 * kBK + csw;
-        double *dstB = smem + ld_st * kSigmaStageDoubles + (kTP + rB0) * kBK + csw;
+        double *dstB = smem + ld_st * kSigmaStageDoubles + (kOldTP + rB0) * kBK + csw;
 #pragma unroll
-        for (int j = 0; j < kTP / 16; ++j) {
+        for (int j = 0; j < kOldTP / 16; ++j) {
           const int nb = (j < nrowA) ? ncol * 8 : 0;
           cp_async_16(dstA + 4 * j * kBK, nb ? srcA + j * stepA : WA, nb);
         }
 #pragma unroll
-        for (int j = 0; j < kTQ / 16; ++j) {
+        for (int j = 0; j < kOldTQ / 16; ++j) {
           const int nb = (j < nrowB) ? ncol * 8 : 0;
           cp_async_16(dstB + 4 * j * kBK, nb ? srcB + j * stepB : WB, nb);
         }
@@ -301,9 +301,9 @@ sigma_accumulate_kernel(const double *__restrict__ WA, int64_t ldA, const double
       // occupation class by bit pattern (no FP64-pipe compare): 1.0 -> occupied term only, +-0.0 -> virtual term only
       const int occ_class = (fbits == 0x3FF0000000000000LL) ? 1 : (((unsigned long long)fbits << 1) == 0ULL ? 0 : 2);
       const double sgn = occ_class == 1 ? 1.0 : -1.0;
-      double d[kTP / 16];
+      double d[kOldTP / 16];
 #pragma unroll
-      for (int j = 0; j < kTP / 16; ++j) d[j] = eps_p[j] - em;
+      for (int j = 0; j < kOldTP / 16; ++j) d[j] = eps_p[j] - em;
       // Omega_s of the next k-tile is fetched one k-tile ahead (a new 128-byte line per k-tile: an L2 round trip)
       double om0n = __ldg(Omega + min(c2, s_c - 1)), om1n = __ldg(Omega + min(c2 + 1, s_c - 1));
 #pragma unroll 1
@@ -315,14 +315,14 @@ sigma_accumulate_kernel(const double *__restrict__ WA, int64_t ldA, const double
         om1n = __ldg(Omega + min(sn + 1, s_c - 1));
         cp_async_wait<kAhead>();                  // this thread's copies of k-tile kt have landed
         double *rowA = smem + st * kSigmaStageDoubles + rA0 * kBK + csw;
-        double2 cur[kTP / 16];
+        double2 cur[kOldTP / 16];
 #pragma unroll
-        for (int j = 0; j < kTP / 16; ++j) cur[j] = *reinterpret_cast<const double2 *>(rowA + 4 * j * kBK);
+        for (int j = 0; j < kOldTP / 16; ++j) cur[j] = *reinterpret_cast<const double2 *>(rowA + 4 * j * kBK);
         if (occ_class != 2) {
           // f_m in {0, 1}: one Lehmann term, x = d + sgn * Omega_s.  The 8 evaluations advance together, stage by
           // stage, so that each dependent step is ONE burst of 8 independent FP64 instructions: the producer warp
           // shares its sub-partition's FP64 pipe with two DMMA streams and pays an arbitration wait per burst.
-          constexpr int E = kTP / 8;
+          constexpr int E = kOldTP / 8;
           double x[E], y[E], r[E];
 #pragma unroll
           for (int e = 0; e < E; ++e) x[e] = fma(sgn, (e & 1) ? om1 : om0, d[e >> 1]);
@@ -339,19 +339,19 @@ sigma_accumulate_kernel(const double *__restrict__ WA, int64_t ldA, const double
 #pragma unroll
           for (int e = 0; e < E; ++e) x[e] = fma(x[e], y[e], x[e]);      // D = q + q t
 #pragma unroll
-          for (int j = 0; j < kTP / 16; ++j) {
+          for (int j = 0; j < kOldTP / 16; ++j) {
             cur[j].x *= x[2 * j];
             cur[j].y *= x[2 * j + 1];
           }
         } else {
 #pragma unroll
-          for (int j = 0; j < kTP / 16; ++j) {
+          for (int j = 0; j < kOldTP / 16; ++j) {
             cur[j].x *= denominator_D<2>(d[j], om0, fo, eta2);
             cur[j].y *= denominator_D<2>(d[j], om1, fo, eta2);
           }
         }
 #pragma unroll
-        for (int j = 0; j < kTP / 16; ++j) *reinterpret_cast<double2 *>(rowA + 4 * j * kBK) = cur[j];
+        for (int j = 0; j < kOldTP / 16; ++j) *reinterpret_cast<double2 *>(rowA + 4 * j * kBK) = cur[j];
         mbar_arrive(full + st);                   // release: the scaled p rows and the landed q rows of this thread
         if (++st == kSigmaStages) st = 0;
       }
@@ -360,7 +360,7 @@ sigma_accumulate_kernel(const double *__restrict__ WA, int64_t ldA, const double
   } else {
     // ------------------------------------------------ consumers
     reg_inc<184>();
-    const SigmaFragMap fm(warp, lane, n_mo - p0, n_mo - q0);
+    const OldSigmaFragMap fm(warp, lane, n_mo - p0, n_mo - q0);
     const bool full_tile = fm.mi_cnt == 4 && fm.nj_cnt == 8;
     double acc[4][8][2];
 #pragma unroll
@@ -373,7 +373,7 @@ sigma_accumulate_kernel(const double *__restrict__ WA, int64_t ldA, const double
     for (int kt = 0; kt < KT; ++kt) {
       mbar_wait(full + st, ph);
       const double *ap = smem + st * kSigmaStageDoubles + (8 * fm.wmi + fm.g) * kBK + fm.t;
-      const double *bp = smem + st * kSigmaStageDoubles + (kTP + 8 * fm.wni + fm.g) * kBK + fm.t;
+      const double *bp = smem + st * kSigmaStageDoubles + (kOldTP + 8 * fm.wni + fm.g) * kBK + fm.t;
       if (full_tile) mma_ktile_sigma<4, 8>(acc, ap, bp, fm.g & 3);
       else mma_ktile_sigma_ragged(acc, ap, bp, fm.g & 3, fm.mi_cnt, fm.nj_cnt);
       __syncwarp();
