@@ -103,6 +103,10 @@ int qsgw_sigma_create(qsgw_sigma_plan **plan, int n_mo, int n_occ, int n_aux, in
  *   Sigma  device [n_mo][n_mo]          OVERWRITTEN; bit-symmetric (Sigma[p][q] == Sigma[q][p])
  * Because Eq. (17) is a plain sum over s, Sigma of a set of poles is the sum of the Sigmas of any
  * partition of it.
+ * Repeated calls with the SAME arguments (pointers, sizes, eta -- the calling pattern of a qsGW loop that
+ * refreshes caller-owned buffers in place) are replayed as one CUDA graph from the third call on, provided the
+ * plan's stream can be captured (not the legacy default stream) and neither profiling nor debug mode is on;
+ * the arithmetic and its order are the same either way.
  */
 int qsgw_sigma_build(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ,
                      const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,

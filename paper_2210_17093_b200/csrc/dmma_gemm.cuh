@@ -230,24 +230,30 @@ struct EpiPairScatter {
   }
 };
 
+// contraction depth of batch b: K, or what is left of k_total when the batches are K-slices of one product
+__device__ __forceinline__ int batch_depth(int K, int k_total, int batch) {
+  return k_total > 0 ? max(0, min(K, k_total - batch * K)) : K;
+}
+
 constexpr size_t kGemmSmemBytes = (size_t)kGemmStages * 2 * kGBK * kLdT * sizeof(double) + 2 * kGemmStages * sizeof(uint64_t);
 
 // C(M x N) = epilogue( sum_k A[k][m] * B[k][n] ),  A stored [K][lda] (m contiguous), B stored [K][ldb] (n contiguous).
 // VECA / VECB = 2 need the operand 16-byte aligned with even leading dimension (and even batch stride); 1 takes anything.
 // nbatch independent problems of the same shape (operands strideA / strideB doubles apart, 0 = shared) share one launch.
+// k_total > 0 makes the batches the K-slices of ONE product (split-K: batch b contracts k in [b K, min((b+1) K, k_total)),
+// the strides advancing K rows, the epilogue storing each slice's partial result).
 // ntm * ntn tiles of 128 x 128 dealt round-robin to the grid; m_fastest picks which tile index varies fastest (the
 // dimension with fewer tiles, so that concurrently running CTAs share operand panels in L2).
 template <int VECA, int VECB, class Epi>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__restrict__ B0, int64_t ldb, int M, int N,
-                    int K, int ntm, int ntn, int m_fastest, int nbatch, int64_t strideA, int64_t strideB, Epi epi0) {
+                    int K, int ntm, int ntn, int m_fastest, int nbatch, int64_t strideA, int64_t strideB, int k_total, Epi epi0) {
   extern __shared__ __align__(16) double smem[];
   double *As = smem;
   double *Bs = smem + kGemmStages * kGBK * kLdT;
   uint64_t *full = reinterpret_cast<uint64_t *>(smem + 2 * kGemmStages * kGBK * kLdT);
   uint64_t *empty = full + kGemmStages;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int KT = (K + kGBK - 1) / kGBK;
   const int tiles_per_batch = ntm * ntn;
   const int ntiles = tiles_per_batch * nbatch;
 
@@ -276,11 +282,13 @@ gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__
       else { tm = t / ntn; tn = t - tm * ntn; }
       const int m0 = tm * kBM, n0 = tn * kBN;
       const double *A = A0 + batch * strideA, *Bm = B0 + batch * strideB;
+      const int Kb = batch_depth(K, k_total, batch);
+      const int KT = (Kb + kGBK - 1) / kGBK;
       for (int kt = 0; kt < KT; ++kt) {
         mbar_wait(empty + st, ph);
         const int k0 = kt * kGBK;
-        load_tile_kmajor<VECA>(As + st * kGBK * kLdT, A + (int64_t)k0 * lda + m0, lda, K - k0, M - m0, A, pt);
-        load_tile_kmajor<VECB>(Bs + st * kGBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, K - k0, N - n0, Bm, pt);
+        load_tile_kmajor<VECA>(As + st * kGBK * kLdT, A + (int64_t)k0 * lda + m0, lda, Kb - k0, M - m0, A, pt);
+        load_tile_kmajor<VECB>(Bs + st * kGBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, Kb - k0, N - n0, Bm, pt);
         cp_async_mbar_arrive_noinc(full + st);
         if (++st == kGemmStages) { st = 0; ph ^= 1; }
       }
@@ -298,6 +306,7 @@ gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__
       else { tm = t / ntn; tn = t - tm * ntn; }
       const int m0 = tm * kBM, n0 = tn * kBN;
       const Epi epi = epi0.for_batch(batch);
+      const int KT = (batch_depth(K, k_total, batch) + kGBK - 1) / kGBK;
       const FragMap fm(warp, lane, M - m0, N - n0);
       const bool full_tile = fm.mi_cnt == 8 && fm.nj_cnt == 4;
       // per-row epilogue context (stage 2: the (p, m) pair of the row), fetched now so its latency hides behind the k loop

@@ -19,7 +19,6 @@
 //   * split-K over m into slot-owned partial tiles (fixed accumulation order, no atomics).
 #pragma once
 #include <cuda.h>
-#include <stdlib.h>
 
 #include "dmma_gemm.cuh"
 
@@ -61,16 +60,15 @@ struct SigmaRings {
   size_t smem_bytes;     // dynamic shared memory to launch with (includes 1 KB of alignment slack and the barriers)
 };
 
-// Ring depths for a tile tq columns wide.  The p ring needs 4 stages (one being read, three being scaled by the three
-// scaling warps); the q ring takes as many stages as fit beside them (at most 4), and what is left deepens the p ring.
+// Ring depths for a tile tq columns wide.  The p ring gets 6 stages if the q ring still has 2 (one being read, three
+// being scaled by the three scaling warps, two landing); the q ring takes the stages that fit beside them (at most 4).
+// Measured at N = 600: a third q stage at the expense of two p stages is slower (583 vs 578 ms per build).
 inline SigmaRings sigma_rings(int tq) {
   SigmaRings r;
   r.b_stage_bytes = 2 * tq * kHalfRowBytes;
   const size_t bar_bytes = 1024;
   const size_t avail = kSigmaSmemBudget - bar_bytes;
-  const char *env = getenv("QSGW_SIGMA_NB");
-  r.nB = (int)((avail - 4 * (size_t)kAStageBytes) / r.b_stage_bytes);
-  if (env) r.nB = atoi(env);
+  r.nB = (int)((avail - 6 * (size_t)kAStageBytes) / r.b_stage_bytes);
   if (r.nB > kMaxBStages) r.nB = kMaxBStages;
   if (r.nB < 2) r.nB = 2;
   r.nA = (int)((avail - (size_t)r.nB * r.b_stage_bytes) / kAStageBytes);
@@ -166,8 +164,8 @@ __device__ __forceinline__ void mma_half_sigma_ragged(double (&acc)[4][8][2], co
   }
 }
 
-// One CTA: output tile (tp, tq) of T, 64 x tq, for the internal states m in [z*m_per_split, ...) and all s_c poles of
-// the chunk.
+// One CTA: output tile (tp, tq) of T, 64 x tq, for the k-tiles of split-K slot z = blockIdx.y: a contiguous range of the
+// (m, 32-pole group) pairs of the chunk (s_c poles, all internal states m).
 //   mapA  tensor map of the left operand (scaled by D)  [m][p][s], box {16 poles, 64 rows, 1}.  qsGW: the w chunk of
 //         stage 2 (both mirrors present); qsMP2 exchange term: the exchange integrals (pi|an)
 //   mapB  tensor map of the right operand, same indexing, box {16 poles, tq rows, 1}.  qsGW: the same array
@@ -177,8 +175,8 @@ __device__ __forceinline__ void mma_half_sigma_ragged(double (&acc)[4][8][2], co
 __global__ void __launch_bounds__(kThreads, 1)
 sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
                         const double *__restrict__ eps, const double *__restrict__ occ, const double *__restrict__ Omega,
-                        int n_mo, int s_c, double eta2, int m_per_split, int ntq, int tq, int nA, int nB,
-                        double *__restrict__ Tpart, int dbg_flags) {
+                        int n_mo, int s_c, double eta2, int nsplit, int ntq, int tq, int nA, int nB,
+                        double *__restrict__ Tpart) {
   extern __shared__ uint8_t smem_raw[];
   // the 128-byte swizzle pattern is a function of the shared-memory ADDRESS: stage bases must be 1024-byte aligned
   // (offset added to the __shared__ array itself, so that the compiler keeps emitting LDS / STS rather than generic accesses)
@@ -196,10 +194,10 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int tp = blockIdx.x / ntq, tqi = blockIdx.x - tp * ntq;
   const int p0 = tp * kTP, q0 = tqi * tq;
-  const int m_begin = blockIdx.y * m_per_split;
-  const int m_end = min(n_mo, m_begin + m_per_split);
+  // split-K: the k-tiles (m, ks), numbered m * KTS + ks, are dealt to the nsplit slots in equal contiguous ranges
   const int KTS = (s_c + kKD - 1) / kKD;         // k-tiles per m
-  const int KT = (m_end - m_begin) * KTS;
+  const int kt_begin = (int)((int64_t)n_mo * KTS * blockIdx.y / nsplit);
+  const int KT = (int)((int64_t)n_mo * KTS * (blockIdx.y + 1) / nsplit) - kt_begin;
 
   if (tid == 0) {
     for (int s = 0; s < nA; ++s) {
@@ -221,9 +219,9 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
     // Its own warp, so that it never waits for the FP64 pipe: the scaling warps below are served only in the gaps of
     // the DMMA streams, and a load that waits behind their arithmetic would stall everybody.
     if (lane == 0) {
-      int a_next = 0, a_st = 0, a_m = m_begin, a_ks = 0;
+      int a_next = 0, a_st = 0, a_m = kt_begin / KTS, a_ks = kt_begin - (kt_begin / KTS) * KTS;
       uint32_t a_ph = 1;                          // a fresh barrier passes a wait on parity 1
-      int b_next = 0, b_st = 0, b_m = m_begin, b_ks = 0;
+      int b_next = 0, b_st = 0, b_m = a_m, b_ks = a_ks;
       uint32_t b_ph = 1;
       // both rings in k-tile order, never blocking on one ring while the other has a free stage
       while (a_next < KT || b_next < KT) {
@@ -268,7 +266,7 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
     uint32_t ph = (sw_id / nA) & 1;
 #pragma unroll 1
     for (int kt = sw_id; kt < KT; kt += kScaleWarps) {
-      const int m = m_begin + kt / KTS, ks = kt - (kt / KTS) * KTS;
+      const int m = (kt_begin + kt) / KTS, ks = (kt_begin + kt) - m * KTS;
       const double em = __ldg(eps + m), fo = __ldg(occ + m);
       const long long fbits = __double_as_longlong(fo);
       // occupation class by bit pattern (no FP64-pipe compare): 1.0 -> occupied term only, +-0.0 -> virtual term only
@@ -282,8 +280,7 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
       }
       mbar_wait(a_raw + st, ph);                  // the raw p rows of this k-tile have landed
       uint8_t *tile = a_ring + st * kAStageBytes;
-      if (dbg_flags & 1) {
-      } else if (occ_class != 2) {
+      if (occ_class != 2) {
         // f_m in {0, 1}: one Lehmann term, x = d + sgn * Omega_s.  8 evaluations (2 rows x 2 halves x 2 poles) advance
         // together, stage by stage, so that each dependent step is ONE burst of 8 independent FP64 instructions.
 #pragma unroll

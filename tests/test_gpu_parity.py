@@ -215,6 +215,37 @@ def test_null_case_and_error_codes():
     pkg.qsgw_sigma_destroy(small_plan)
 
 
+def test_repeated_build_on_a_side_stream_replays_as_a_cuda_graph():
+    """Identical calls on a capturable stream: the third call on is one CUDA graph launch; results are bitwise those of
+    the launch-by-launch path, and they follow the CONTENTS of the caller's buffers (refreshed in place)."""
+    pkg = _pkg()
+    cfg = qi.custom_config(150, 11, 70, n_pole=300, s_block=128, seed=77)
+    inp = qi.make_inputs(cfg)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        B, eps, occ, Om, Z = _to_dev(inp)
+        plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, cfg.n_pole, cfg.s_block, stream=stream)
+        S = torch.empty((cfg.n_mo, cfg.n_mo), dtype=torch.float64, device="cuda")
+        outs = []
+        for _ in range(4):
+            pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta, S)
+            stream.synchronize()
+            outs.append(S.clone())
+        st = pkg.qsgw_sigma_get_stats(plan)
+        assert st["builds"] == 4 and st["poles"] == 4 * cfg.n_pole
+        assert all(torch.equal(outs[0], o) for o in outs[1:])
+        _assert_parity(outs[3], _ref_sigma(cfg, inp))
+        Z.mul_(2.0)                                              # same pointers, new contents: the graph must see them
+        pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta, S)
+        stream.synchronize()
+        assert torch.equal(S, 4.0 * outs[0])
+        Z.mul_(0.5)
+        S2 = pkg.qsgw_sigma_build(plan, B, eps, occ, Om, Z, cfg.eta)        # other output pointer: launch by launch again
+        stream.synchronize()
+        assert torch.equal(S2, outs[0])
+        pkg.qsgw_sigma_destroy(plan)
+
+
 def test_debug_mode_checks_the_device_side_preconditions():
     """occ in [0,1], Omega > 0 and B symmetric are documented preconditions, verified only in debug mode."""
     pkg = _pkg()
