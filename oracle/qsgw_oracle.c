@@ -439,3 +439,60 @@ void qsgw_oracle_set_num_threads(int n) {
   (void)n;
 #endif
 }
+
+/* ---- row 8(f).4, second half: the Casida / RPA step that produces Omega and Z = X + Y ---------------------------------
+ * Eqs. (12)-(14), closed shell, real orbitals, RI integrals (ia|jb) = sum_P B[P][i][a] B[P][j][b]
+ * (PAPER.md:120), direct RPA (no exchange kernel).  Spin-adapted singlet block: A = Delta + 2K, B = 2K with
+ * Delta_ia = eps[a] - eps[i] (diagonal) and K[ia][jb] = (ia|jb), hence
+ *   A - B = Delta (diagonal),   A + B = Delta + 4 K.
+ * Sign reading: Eqs. (13)-(14) print the Coulomb terms with a minus sign; the RPA polarizability
+ * chi = chi0 + chi0 v chi of Eq. (11) gives A = Delta + K, B = K per spin pair, and only that sign keeps every Omega_s real
+ * and >= min Delta > 0 for the positive semidefinite RI kernel -- the precondition Omega > 0 of the Sigma build.
+ * For real orbitals Eq. (12) reduces to the symmetric problem (the standard Casida reduction)
+ *   C xi_s = Omega_s^2 xi_s,   C = (A-B)^(1/2) (A+B) (A-B)^(1/2),   C[ia][jb] = Delta_ia^2 delta + 4 sqrt(Delta_ia) K[ia][jb] sqrt(Delta_jb)
+ *   X^s + Y^s = (A-B)^(1/2) xi_s / sqrt(Omega_s)            (normalisation (X+Y)^T (X-Y) = 1, xi_s orthonormal)
+ * This function writes C (step before the eigensolve); qsgw_oracle_casida_z does the step after it.  The symmetric
+ * eigensolve in between is a library routine (numpy.linalg.eigh in qsgw_oracle.py).  Composite index ia = i*v + (a-o).
+ * C is n_ov x n_ov row-major.  Returns 0 / -1. */
+int qsgw_oracle_casida_matrix(int N, int o, int naux, const double *B, const double *eps, double *C) {
+  if (N < 2 || o < 1 || o >= N || naux < 1) return -1;
+  const int v = N - o;
+  const size_t nov = (size_t)o * v;
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < o; ++i) {
+    for (int a = o; a < N; ++a) {
+      const size_t ia = (size_t)i * v + (a - o);
+      const double d_ia = eps[a] - eps[i];
+      for (int j = 0; j < o; ++j) {
+        for (int b = o; b < N; ++b) {
+          const size_t jb = (size_t)j * v + (b - o);
+          const double d_jb = eps[b] - eps[j];
+          double k = 0.0;                                                        /* (ia|jb) */
+          for (int P = 0; P < naux; ++P) k += B[((size_t)P * N + i) * N + a] * B[((size_t)P * N + j) * N + b];
+          C[ia * nov + jb] = (ia == jb ? d_ia * d_ia : 0.0) + 4.0 * sqrt(d_ia) * k * sqrt(d_jb);
+        }
+      }
+    }
+  }
+  return 0;
+}
+
+/* After the eigensolve: lambda[s] (eigenvalues of C, = Omega_s^2) and xi[ia][s] (orthonormal eigenvectors in the columns,
+ * leading dimension ldxi) -> Omega[s] = sqrt(lambda[s]),  Z[ia][s] = sqrt(Delta_ia) * xi[ia][s] / sqrt(Omega[s]).
+ * n_pole <= n_ov columns are converted.  Z is [n_ov][ldz].  Returns 0, or -1 on bad arguments or a non-positive lambda. */
+int qsgw_oracle_casida_z(int N, int o, const double *eps, int64_t n_pole, const double *lambda, const double *xi,
+                         int64_t ldxi, double *Omega, double *Z, int64_t ldz) {
+  if (N < 2 || o < 1 || o >= N || n_pole < 1 || ldxi < n_pole || ldz < n_pole) return -1;
+  const int v = N - o;
+  for (int64_t s = 0; s < n_pole; ++s) {
+    if (!(lambda[s] > 0.0)) return -1;
+    Omega[s] = sqrt(lambda[s]);
+  }
+  for (int i = 0; i < o; ++i)
+    for (int a = o; a < N; ++a) {
+      const size_t ia = (size_t)i * v + (a - o);
+      const double sd = sqrt(eps[a] - eps[i]);
+      for (int64_t s = 0; s < n_pole; ++s) Z[ia * ldz + s] = sd * xi[ia * ldxi + s] / sqrt(Omega[s]);
+    }
+  return 0;
+}

@@ -62,6 +62,10 @@ def _load():
         lib.qsgw_oracle_mp2_states.restype = ctypes.c_int
         lib.qsgw_oracle_mp2_states.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, ctypes.c_double, ctypes.c_int,
                                                ctypes.c_int, ip, dp]
+        lib.qsgw_oracle_casida_matrix.restype = ctypes.c_int
+        lib.qsgw_oracle_casida_matrix.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp]
+        lib.qsgw_oracle_casida_z.restype = ctypes.c_int
+        lib.qsgw_oracle_casida_z.argtypes = [ctypes.c_int, ctypes.c_int, dp, i64, dp, dp, i64, dp, dp, i64]
         lib.qsgw_oracle_ao_to_mo.restype = ctypes.c_int
         lib.qsgw_oracle_ao_to_mo.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp]
         _lib = lib
@@ -248,3 +252,45 @@ def mp2(B, eps, occ, eta: float, n_occ: int, sox_only: bool = False, states=None
     if rc != 0:
         raise RuntimeError(f"qsgw_oracle_mp2 failed with {rc}")
     return out
+
+
+def casida_matrix(B, eps, n_occ: int):
+    """C = (A-B)^(1/2) (A+B) (A-B)^(1/2) of the closed-shell direct-RPA Casida problem, Eqs. (12)-(14)
+    with RI integrals: C[ia,jb] = Delta_ia^2 delta + 4 sqrt(Delta_ia) (ia|jb) sqrt(Delta_jb).  Returns [n_ov, n_ov]."""
+    B = _f64(B)
+    naux, N, N2 = B.shape
+    if N != N2:
+        raise ValueError("B must be [naux, N, N]")
+    eps = _f64(eps, (N,))
+    nov = n_occ * (N - n_occ)
+    C = np.empty((nov, nov))
+    rc = _load().qsgw_oracle_casida_matrix(N, n_occ, naux, _dp(B), _dp(eps), _dp(C))
+    if rc != 0:
+        raise RuntimeError(f"qsgw_oracle_casida_matrix failed with {rc}")
+    return C
+
+
+def casida_z(eps, n_occ: int, lam, xi):
+    """After the eigensolve: Omega = sqrt(lambda), Z[ia,s] = sqrt(Delta_ia) xi[ia,s] / sqrt(Omega_s)  (X + Y of Eq. (18))."""
+    eps = _f64(eps)
+    N = eps.shape[0]
+    lam = _f64(lam)
+    xi = _f64(xi)
+    nov = n_occ * (N - n_occ)
+    n_pole = lam.shape[0]
+    if xi.shape != (nov, n_pole):
+        raise ValueError(f"xi must be [{nov}, {n_pole}]")
+    Omega = np.empty(n_pole)
+    Z = np.empty((nov, n_pole))
+    rc = _load().qsgw_oracle_casida_z(N, n_occ, _dp(eps), n_pole, _dp(lam), _dp(xi), n_pole, _dp(Omega), _dp(Z), n_pole)
+    if rc != 0:
+        raise RuntimeError(f"qsgw_oracle_casida_z failed with {rc} (non-positive eigenvalue?)")
+    return Omega, Z
+
+
+def casida(B, eps, n_occ: int):
+    """The whole Casida / RPA step, Eqs. (12)-(14): (Omega [n_ov] ascending, Z = X + Y [n_ov, n_ov]).  Plain loops for C and
+    for the back-transformation; the symmetric eigensolve between them is numpy.linalg.eigh (a library routine as a step)."""
+    C = casida_matrix(B, eps, n_occ)
+    lam, xi = np.linalg.eigh(C)
+    return casida_z(eps, n_occ, lam, xi)
