@@ -707,6 +707,86 @@ def run_gpu_mp2(args):
     return 0
 
 
+def run_gpu_casida(args):
+    """--path casida: row 8(f).4, the two library steps of the Casida / RPA solve around the eigensolve.
+    value = FP64 TFLOP/s of qsgw_casida_matrix on the algorithmic minimum 2 * [n_ov (n_ov + 1) / 2] * naux flops (the
+    symmetric half of K = Bov^T Bov); the back-transformation qsgw_casida_z is reported against the HBM roofline
+    (16 bytes per element of Z: xi read once, Z written once).  The eigensolve between them is a library call (cuSOLVER
+    through torch.linalg.eigh), timed for context only up to `medium`."""
+    import torch
+    import qsgw_inputs as qi
+    import paper_2210_17093_b200 as pkg
+
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("--path casida is a single-GPU measurement")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    cfg = qi.CONFIGS[args.workload]
+    if cfg.name == "xl":
+        raise SystemExit("--path casida: C of xl is 130 GB; use tiny..large")
+    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak, peak_src, pk = fp64_peak_tflops(nsm)
+    B = qi.make_B(cfg, dev)
+    eps = qi.make_eps(cfg).to(dev)
+    n_ov = cfg.n_ov
+    work = torch.empty(pkg.qsgw_casida_work_doubles(cfg.n_mo, cfg.n_occ, cfg.n_aux), dtype=torch.float64, device=dev)
+    C = torch.empty((n_ov, n_ov), dtype=torch.float64, device=dev)
+
+    def timed_loop(fn):
+        for _ in range(args.warmup):
+            fn()
+        torch.cuda.synchronize()
+        evs = []
+        for _ in range(args.steps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            evs.append((e0, e1))
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in evs) / args.steps
+
+    with ClockSampler(0) as clocks:
+        ms_c = timed_loop(lambda: pkg.qsgw_casida_matrix(B, eps, cfg.n_occ, C, work))
+    flops = 2.0 * (n_ov * (n_ov + 1) / 2) * cfg.n_aux
+    val = flops / (ms_c * 1e-3) / 1e12
+    assert torch.isfinite(C).all() and torch.equal(C, C.T)
+    eigh_ms = None
+    if n_ov <= 10400:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); lam, xi = torch.linalg.eigh(C); e1.record(); torch.cuda.synchronize()
+        eigh_ms = e0.elapsed_time(e1)
+        xi = xi.contiguous()
+    else:       # a stand-in with the right shapes for the back-transformation's timing (values do not matter for it)
+        lam = torch.rand(n_ov, dtype=torch.float64, device=dev) + 0.5
+        xi = C
+    Om = torch.empty(n_ov, dtype=torch.float64, device=dev)
+    Z = torch.empty((n_ov, n_ov), dtype=torch.float64, device=dev) if n_ov <= 10400 else work.new_empty((n_ov, n_ov))
+    ms_z = timed_loop(lambda: pkg.qsgw_casida_z(eps, cfg.n_occ, lam, xi, Om, Z))
+    hbm = float(pk.get("hbm_gbs", 6650.0))
+    z_gbs = 16.0 * n_ov * n_ov / (ms_z * 1e-3) / 1e9
+    out = {"metric": "casida_matrix_fp64_tflops", "value": val, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms_c, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "path": "casida (SURVEY.md 8(f).4)", "config": _config_dict(cfg, args, extra={"n_ov": n_ov, "flops_symmetric_half": flops}),
+           "roofline": {"bound": "tensor", "kernel": "gemm_tn_dmma_kernel<2,2,EpiCasida> (upper-triangle tiles)", "achieved": val, "peak": peak,
+                        "unit": UNIT, "frac": val / peak, "launches": args.steps, "avg_launch_ms": ms_c, "traffic": None,
+                        "peak_source": f"FP64 pipe rate at max SM clock ({peak_src})"},
+           "casida_z": {"ms": ms_z, "achieved_gbs": z_gbs, "peak_gbs": hbm, "frac": z_gbs / hbm, "bound": "hbm",
+                        "bytes_per_element": 16, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})"},
+           "eigensolve_library_ms": eigh_ms, "gpu_launches": 3 * args.steps, "clocks": clocks.summary(),
+           "e2e": {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                   "how": "B and C stay on the device between the AO->MO transform, the eigensolve and the Sigma build"}}
+    if not args.no_cpu_baseline and n_ov <= 2000:
+        import oracle
+        t0 = time.perf_counter()
+        oracle.casida_matrix(B.cpu().numpy(), eps.cpu().numpy(), cfg.n_occ)
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": flops / dt / 1e12, "unit": UNIT + " (GPU flop model / oracle time)", "cores": oracle.num_threads(),
+                               "kind": "oracle", "sample": f"whole C of '{cfg.name}' ({dt:.1f} s)"}
+    print(json.dumps(out), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -722,7 +802,7 @@ def main():
     ap.add_argument("--e2e-warmup", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-poles", type=int, default=0, help="poles in the oracle's timed sample (0 = auto, ~20 s)")
-    ap.add_argument("--path", default="sigma", choices=["sigma", "diag", "aomo", "mp2"],
+    ap.add_argument("--path", default="sigma", choices=["sigma", "diag", "aomo", "mp2", "casida"],
                     help="sigma: the qsGW Sigma^c build (the bench contract); diag: the G0W0 diagonal on a frequency grid")
     ap.add_argument("--n-omega", type=int, default=64, help="grid points of --path diag")
     args = ap.parse_args()
@@ -736,6 +816,8 @@ def main():
         return run_gpu_aomo(args)
     if args.path == "mp2":
         return run_gpu_mp2(args)
+    if args.path == "casida":
+        return run_gpu_casida(args)
     return run_gpu(args)
 
 

@@ -210,6 +210,36 @@ size_t qsgw_ri_ao_to_mo_work_doubles(int n_aux, int n_ao, int n_mo);
  */
 int qsgw_sigma_pole_slice(int64_t n_pole, int n_ranks, int rank, int64_t *s0, int64_t *n);
 
+/*
+ * Row 8(f).4, second half: the Casida / RPA step that produces the Omega and Z arguments of the build (Eqs. (12)-(14),
+ * PAPER.md:130-136; "the next bottleneck").  Closed shell, real orbitals, direct RPA, RI integrals
+ * (ia|jb) = sum_P B[P][i][a] B[P][j][b]: A - B = Delta (diagonal, Delta_ia = eps[a] - eps[i]), A + B = Delta + 4 K, and
+ * Eq. (12) reduces to the symmetric problem C xi_s = Omega_s^2 xi_s with
+ *   C[ia][jb] = Delta_ia^2 delta_{ia,jb} + 4 sqrt(Delta_ia) (ia|jb) sqrt(Delta_jb),   X^s + Y^s = sqrt(Delta) xi_s / sqrt(Omega_s).
+ * (Sign reading: Eqs. (13)-(14) print the Coulomb terms with a minus sign; + is taken, the sign that follows
+ * from Eq. (11) and keeps Omega real.)  The library does the two steps around the eigensolve; the dense symmetric
+ * eigensolve itself is NOT part of this library (callers use a library routine, e.g. cuSOLVER through torch.linalg.eigh).
+ *
+ * qsgw_casida_matrix: C from B and eps -- one gather kernel and one FP64 tensor-core GEMM over the auxiliary index
+ * (upper-triangle tiles only, mirrored in the epilogue: n_ov (n_ov + 128) naux flops); C is bit-symmetric.
+ *   B     device [n_aux][n_mo][n_mo]; only the occupied-virtual block B[P][i][a], i < n_occ <= a, is read
+ *   eps   device [n_mo]; eps[a] > eps[i] for every pair (else C holds NaN)
+ *   work  device, qsgw_casida_work_doubles(n_mo, n_occ, n_aux) doubles, 16-byte aligned; caller-owned scratch
+ *   C     device [n_ov][ldc], n_ov = n_occ * (n_mo - n_occ), row / column ia = i * n_virt + (a - n_occ); OVERWRITTEN
+ * qsgw_casida_z: after the eigensolve, for the first n_pole eigenpairs handed in,
+ *   Omega[s] = sqrt(lambda[s]),   Z[ia][s] = sqrt(Delta_ia) * xi[ia][s] / sqrt(Omega[s])
+ *   lambda device [n_pole] eigenvalues of C (> 0);  xi device [n_ov][ldxi], eigenvector s in column s (orthonormal)
+ *   Omega  device [n_pole], Z device [n_ov][ldz]: OVERWRITTEN; they are the Omega / Z arguments of qsgw_sigma_build.
+ * Both are asynchronous on cuda_stream (a cudaStream_t or NULL) and need no plan.
+ * Errors: INVALID_ARG for NULL pointers, sizes out of range, leading dimensions too small, a misaligned work buffer;
+ * CUDA if no sm_100 device or a launch fails (message: qsgw_sigma_last_error(NULL)).
+ */
+size_t qsgw_casida_work_doubles(int n_mo, int n_occ, int n_aux);
+int qsgw_casida_matrix(const double *B, const double *eps, int n_mo, int n_occ, int n_aux, double *work, double *C,
+                       int64_t ldc, void *cuda_stream);
+int qsgw_casida_z(const double *eps, int n_mo, int n_occ, const double *lambda, const double *xi, int64_t ldxi,
+                  int64_t n_pole, double *Omega, double *Z, int64_t ldz, void *cuda_stream);
+
 /* Free the workspace and the plan.  Synchronises the plan's stream first.  NULL is accepted. */
 int qsgw_sigma_destroy(qsgw_sigma_plan *plan);
 

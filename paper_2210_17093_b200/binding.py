@@ -29,7 +29,7 @@ EXPORTS = (
     "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
     "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_mp2_direct_build", "qsgw_mp2_build", "qsgw_ri_ao_to_mo", "qsgw_ri_ao_to_mo_work_doubles", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
     "qsgw_sigma_limit_pole_batch", "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_set_debug", "qsgw_sigma_version",
-    "qsgw_sigma_pole_slice",
+    "qsgw_sigma_pole_slice", "qsgw_casida_work_doubles", "qsgw_casida_matrix", "qsgw_casida_z",
 )
 
 
@@ -103,6 +103,12 @@ def load_library() -> ctypes.CDLL:
         lib.qsgw_sigma_get_stats.argtypes = [vp, ctypes.POINTER(qsgw_sigma_stats), ci]
         lib.qsgw_sigma_pole_slice.restype = ci
         lib.qsgw_sigma_pole_slice.argtypes = [i64, ci, ci, ctypes.POINTER(i64), ctypes.POINTER(i64)]
+        lib.qsgw_casida_work_doubles.restype = ctypes.c_size_t
+        lib.qsgw_casida_work_doubles.argtypes = [ci, ci, ci]
+        lib.qsgw_casida_matrix.restype = ci
+        lib.qsgw_casida_matrix.argtypes = [dp, dp, ci, ci, ci, dp, dp, i64, vp]
+        lib.qsgw_casida_z.restype = ci
+        lib.qsgw_casida_z.argtypes = [dp, ci, ci, dp, dp, i64, i64, dp, dp, i64, vp]
         lib.qsgw_sigma_set_debug.restype = ci
         lib.qsgw_sigma_set_debug.argtypes = [vp, ci]
         lib.qsgw_sigma_version.restype = ci
@@ -342,6 +348,59 @@ def qsgw_sigma_pole_slice(n_pole: int, n_ranks: int, rank: int):
     s0, n = ctypes.c_int64(), ctypes.c_int64()
     _check(load_library().qsgw_sigma_pole_slice(int(n_pole), int(n_ranks), int(rank), ctypes.byref(s0), ctypes.byref(n)), None)
     return int(s0.value), int(n.value)
+
+
+def qsgw_casida_work_doubles(n_mo: int, n_occ: int, n_aux: int) -> int:
+    return int(load_library().qsgw_casida_work_doubles(int(n_mo), int(n_occ), int(n_aux)))
+
+
+def qsgw_casida_matrix(B: torch.Tensor, eps: torch.Tensor, n_occ: int, C: Optional[torch.Tensor] = None,
+                       work: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """C = (A-B)^(1/2) (A+B) (A-B)^(1/2) of the closed-shell RPA Casida problem (Eqs. (12)-(14)); [n_ov, n_ov], bit-symmetric."""
+    if B.dim() != 3 or B.shape[1] != B.shape[2] or not B.is_contiguous() or not eps.is_contiguous():
+        raise ValueError("need contiguous B [n_aux, n_mo, n_mo] and eps [n_mo]")
+    n_aux, n_mo = int(B.shape[0]), int(B.shape[1])
+    n_ov = n_occ * (n_mo - n_occ)
+    if C is None:
+        C = torch.empty((n_ov, n_ov), dtype=torch.float64, device=B.device)
+    if C.dim() != 2 or tuple(C.shape) != (n_ov, n_ov) or C.stride(1) != 1:
+        raise ValueError(f"C must be [{n_ov}, {n_ov}] with unit column stride")
+    need = qsgw_casida_work_doubles(n_mo, n_occ, n_aux)
+    if work is None:
+        work = torch.empty(need, dtype=torch.float64, device=B.device)
+    if work.numel() < need or not work.is_contiguous():
+        raise ValueError(f"work needs {need} contiguous doubles")
+    if stream is None:
+        stream = torch.cuda.current_stream(B.device)
+    for t in (B, eps, C, work):
+        t.record_stream(stream)
+    rc = load_library().qsgw_casida_matrix(_dev(B, "B"), _dev(eps, "eps", (n_mo,)), n_mo, int(n_occ), n_aux, _dev(work, "work"),
+                                           _dev(C, "C"), int(C.stride(0)), ctypes.c_void_p(stream.cuda_stream))
+    _check(rc, None)
+    return C
+
+
+def qsgw_casida_z(eps: torch.Tensor, n_occ: int, lam: torch.Tensor, xi: torch.Tensor, Omega: Optional[torch.Tensor] = None,
+                  Z: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None):
+    """(Omega, Z): Omega = sqrt(lambda), Z[ia, s] = sqrt(Delta_ia) xi[ia, s] / sqrt(Omega_s) for the eigenpairs handed in."""
+    n_mo = int(eps.shape[0])
+    n_ov = n_occ * (n_mo - n_occ)
+    n_pole = int(lam.shape[0])
+    if xi.dim() != 2 or tuple(xi.shape) != (n_ov, n_pole) or xi.stride(1) != 1 or not lam.is_contiguous():
+        raise ValueError(f"xi must be [{n_ov}, {n_pole}] with unit column stride (eigenvectors in the columns), lambda contiguous")
+    if Omega is None:
+        Omega = torch.empty(n_pole, dtype=torch.float64, device=xi.device)
+    if Z is None:
+        Z = torch.empty((n_ov, n_pole), dtype=torch.float64, device=xi.device)
+    if stream is None:
+        stream = torch.cuda.current_stream(xi.device)
+    for t in (eps, lam, xi, Omega, Z):
+        t.record_stream(stream)
+    rc = load_library().qsgw_casida_z(_dev(eps, "eps"), n_mo, int(n_occ), _dev(lam, "lambda"), _dev(xi, "xi"), int(xi.stride(0)) if n_ov > 1 else n_pole,
+                                      n_pole, _dev(Omega, "Omega", (n_pole,)), _dev(Z, "Z", (n_ov, n_pole)), int(Z.stride(0)) if n_ov > 1 else n_pole,
+                                      ctypes.c_void_p(stream.cuda_stream))
+    _check(rc, None)
+    return Omega, Z
 
 
 def qsgw_sigma_version() -> int:

@@ -230,6 +230,44 @@ struct EpiPairScatter {
   }
 };
 
+// Tile t of a batch -> (tm, tn).  tri: only the tiles with tm <= tn of a square tile grid are enumerated (symmetric
+// products: t = tn (tn + 1) / 2 + tm); otherwise all ntm x ntn tiles, the index named by m_fastest varying fastest.
+__device__ __forceinline__ void decode_tile(int t, int ntm, int ntn, int m_fastest, int tri, int &tm, int &tn) {
+  if (tri) {
+    tn = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
+    while (tn * (tn + 1) / 2 > t) --tn;
+    while ((tn + 1) * (tn + 2) / 2 <= t) ++tn;
+    tm = t - tn * (tn + 1) / 2;
+  } else if (m_fastest) {
+    tn = t / ntm; tm = t - tn * ntm;
+  } else {
+    tm = t / ntn; tn = t - tm * ntn;
+  }
+}
+
+// Casida matrix (Eqs. (12)-(14)): C[r][c] = 4 sqrt(Delta_r) acc sqrt(Delta_c) + (r == c) Delta_r^2 from
+// acc = K[r][c] = (ia|jb).  Launched over the upper-triangle tiles only; off-diagonal tiles also store the mirror element
+// C[c][r].  The scale factor is formed as (4 acc) * (sqrt(Delta_r) sqrt(Delta_c)) -- symmetric in r <-> c to the last bit.
+struct EpiCasida {
+  double *C;
+  int64_t ldc;
+  const double *sqd;   // [n_ov] sqrt(Delta)
+  const double *d;     // [n_ov] Delta
+  using RowCtx = double;
+  __device__ __forceinline__ EpiCasida for_batch(int) const { return *this; }
+  __device__ __forceinline__ RowCtx row_ctx(int row) const { return __ldg(sqd + row); }
+  __device__ __forceinline__ void one(double sr, int row, int col, double v) const {
+    double c = (4.0 * v) * (sr * __ldg(sqd + col));
+    if (row == col) { const double dr = __ldg(d + row); c += dr * dr; }
+    C[(int64_t)row * ldc + col] = c;
+    if ((row / kBM) != (col / kBN)) C[(int64_t)col * ldc + row] = c;
+  }
+  __device__ __forceinline__ void operator()(RowCtx sr, int row, int col, double v0, double v1, int ncols) const {
+    one(sr, row, col, v0);
+    if (col + 1 < ncols) one(sr, row, col + 1, v1);
+  }
+};
+
 // contraction depth of batch b: K, or what is left of k_total when the batches are K-slices of one product
 __device__ __forceinline__ int batch_depth(int K, int k_total, int batch) {
   return k_total > 0 ? max(0, min(K, k_total - batch * K)) : K;
@@ -247,14 +285,14 @@ constexpr size_t kGemmSmemBytes = (size_t)kGemmStages * 2 * kGBK * kLdT * sizeof
 template <int VECA, int VECB, class Epi>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__restrict__ B0, int64_t ldb, int M, int N,
-                    int K, int ntm, int ntn, int m_fastest, int nbatch, int64_t strideA, int64_t strideB, int k_total, Epi epi0) {
+                    int K, int ntm, int ntn, int m_fastest, int nbatch, int64_t strideA, int64_t strideB, int k_total, int tri, Epi epi0) {
   extern __shared__ __align__(16) double smem[];
   double *As = smem;
   double *Bs = smem + kGemmStages * kGBK * kLdT;
   uint64_t *full = reinterpret_cast<uint64_t *>(smem + 2 * kGemmStages * kGBK * kLdT);
   uint64_t *empty = full + kGemmStages;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tiles_per_batch = ntm * ntn;
+  const int tiles_per_batch = tri ? ntn * (ntn + 1) / 2 : ntm * ntn;
   const int ntiles = tiles_per_batch * nbatch;
 
   if (tid == 0) {
@@ -278,8 +316,7 @@ gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       const int batch = tile / tiles_per_batch, t = tile - batch * tiles_per_batch;
       int tm, tn;
-      if (m_fastest) { tn = t / ntm; tm = t - tn * ntm; }
-      else { tm = t / ntn; tn = t - tm * ntn; }
+      decode_tile(t, ntm, ntn, m_fastest, tri, tm, tn);
       const int m0 = tm * kBM, n0 = tn * kBN;
       const double *A = A0 + batch * strideA, *Bm = B0 + batch * strideB;
       const int Kb = batch_depth(K, k_total, batch);
@@ -302,8 +339,7 @@ gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       const int batch = tile / tiles_per_batch, t = tile - batch * tiles_per_batch;
       int tm, tn;
-      if (m_fastest) { tn = t / ntm; tm = t - tn * ntm; }
-      else { tm = t / ntn; tn = t - tm * ntn; }
+      decode_tile(t, ntm, ntn, m_fastest, tri, tm, tn);
       const int m0 = tm * kBM, n0 = tn * kBN;
       const Epi epi = epi0.for_batch(batch);
       const int KT = (batch_depth(K, k_total, batch) + kGBK - 1) / kGBK;

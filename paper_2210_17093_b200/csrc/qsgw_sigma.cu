@@ -188,6 +188,7 @@ cudaError_t configure_kernels_for_device(int dev) {
   set(allow_smem(gemm_tn_dmma_kernel<1, 2, EpiStore>, kGemmSmemBytes));
   set(allow_smem(gemm_tn_dmma_kernel<1, 1, EpiStore>, kGemmSmemBytes));
   set(allow_smem(gemm_tn_dmma_kernel<2, 2, EpiPairScatter>, kGemmSmemBytes));
+  set(allow_smem(gemm_tn_dmma_kernel<2, 2, EpiCasida>, kGemmSmemBytes));
   set(allow_smem(sigma_accumulate_kernel, kSigmaSmemBudget + 1024));
   set(allow_smem(sigma_diag_kernel, kDiagSmemMax));
   if (e == cudaSuccess && dev >= 0 && dev < kMaxDevices) g_attr_done[dev] = true;
@@ -219,7 +220,7 @@ int launch_gemm_on(qsgw_sigma_plan *p, cudaStream_t stream, int num_sms, const d
   // persistent: one CTA per SM walks the tiles round-robin; the dimension with fewer tiles varies fastest, so that the
   // CTAs running at the same time share its few operand panels in L2
   kern<<<std::min(ntm * ntn * nbatch, num_sms), kThreads, kGemmSmemBytes, stream>>>(
-      A, lda, Bm, ldb, M, N, K, ntm, ntn, ntm <= ntn ? 1 : 0, nbatch, strideA, strideB, k_total, epi);
+      A, lda, Bm, ldb, M, N, K, ntm, ntn, ntm <= ntn ? 1 : 0, nbatch, strideA, strideB, k_total, 0, epi);
   QSGW_CUDA(p, cudaGetLastError());
   return QSGW_SIGMA_OK;
 }
@@ -899,6 +900,77 @@ int qsgw_ri_ao_to_mo(const double *B_ao, const double *C, int n_aux, int n_ao, i
                 : launch_gemm_on<2, 1>(nullptr, stream, sms, work, ldt, C, n_mo, n_mo, n_mo, n_ao, epi, n_aux, sT, 0);
     if (rc) return rc;
   }
+  return QSGW_SIGMA_OK;
+}
+
+size_t qsgw_casida_work_doubles(int n_mo, int n_occ, int n_aux) {
+  if (n_mo < 2 || n_occ < 1 || n_occ >= n_mo || n_aux < 1) return 0;
+  const size_t ld_ov = (size_t)round_up((int64_t)n_occ * (n_mo - n_occ), 2);
+  return ((size_t)n_aux + 2) * ld_ov;
+}
+
+namespace {
+int device_for_free_function(int *dev, int *sms) {
+  int major = 0;
+  cudaError_t e = cudaGetDevice(dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, *dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, *dev);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, QSGW_SIGMA_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
+  }
+  if (major != 10) return fail(nullptr, QSGW_SIGMA_ERR_CUDA, "this library is built for sm_100a (B200) only");
+  if ((e = configure_kernels_for_device(*dev)) != cudaSuccess)
+    return fail(nullptr, QSGW_SIGMA_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+  return QSGW_SIGMA_OK;
+}
+}  // namespace
+
+int qsgw_casida_matrix(const double *B, const double *eps, int n_mo, int n_occ, int n_aux, double *work, double *C,
+                       int64_t ldc, void *cuda_stream) {
+  if (!B || !eps || !work || !C) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "casida_matrix: NULL argument");
+  if (n_mo < 2 || n_occ < 1 || n_occ >= n_mo || n_aux < 1)
+    return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "casida_matrix: need n_mo >= 2, 1 <= n_occ < n_mo, n_aux >= 1");
+  const int64_t n_ov = (int64_t)n_occ * (n_mo - n_occ);
+  if (n_ov > INT32_MAX / 2 || ldc < n_ov) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "casida_matrix: ldc < n_occ*n_virt (or too large)");
+  if (reinterpret_cast<uintptr_t>(work) & 15) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "casida_matrix: work must be 16-byte aligned");
+  int dev = 0, sms = 0, rc;
+  if ((rc = device_for_free_function(&dev, &sms))) return rc;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const int64_t ld_ov = round_up(n_ov, 2);
+  double *Bov = work, *d = work + (size_t)n_aux * ld_ov, *sqd = d + ld_ov;
+  casida_gather_kernel<<<dim3((unsigned)((n_ov + 255) / 256), n_aux + 1), 256, 0, stream>>>(B, eps, n_mo, n_occ, n_aux, Bov, ld_ov, d, sqd);
+  QSGW_CUDA(nullptr, cudaGetLastError());
+  // K = Bov^T Bov over the auxiliary index, upper-triangle tiles only; the epilogue scales, adds Delta^2 and mirrors
+  const int nt = (int)((n_ov + kBM - 1) / kBM);
+  const int64_t ntiles = (int64_t)nt * (nt + 1) / 2;
+  if (ntiles > INT32_MAX) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "casida_matrix: tile grid too large");
+  EpiCasida epi{C, ldc, sqd, d};
+  gemm_tn_dmma_kernel<2, 2, EpiCasida><<<(int)std::min<int64_t>(ntiles, sms), kThreads, kGemmSmemBytes, stream>>>(
+      Bov, ld_ov, Bov, ld_ov, (int)n_ov, (int)n_ov, n_aux, nt, nt, 0, 1, 0, 0, 0, 1, epi);
+  QSGW_CUDA(nullptr, cudaGetLastError());
+  return QSGW_SIGMA_OK;
+}
+
+int qsgw_casida_z(const double *eps, int n_mo, int n_occ, const double *lambda, const double *xi, int64_t ldxi,
+                  int64_t n_pole, double *Omega, double *Z, int64_t ldz, void *cuda_stream) {
+  if (!eps || !lambda || !xi || !Omega || !Z) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "casida_z: NULL argument");
+  if (n_mo < 2 || n_occ < 1 || n_occ >= n_mo) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "casida_z: need n_mo >= 2, 1 <= n_occ < n_mo");
+  const int64_t n_ov = (int64_t)n_occ * (n_mo - n_occ);
+  if (n_pole < 1 || n_pole > n_ov || ldxi < n_pole || ldz < n_pole)
+    return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "casida_z: need 1 <= n_pole <= n_occ*n_virt, ldxi >= n_pole, ldz >= n_pole");
+  int dev = 0, sms = 0, rc;
+  if ((rc = device_for_free_function(&dev, &sms))) return rc;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const int64_t row_blocks = (n_ov + 7) / 8;
+  if (row_blocks + 1 > 65535)     // gridDim.y limit
+    return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "casida_z: n_occ*n_virt above 524272 is not supported");
+  const dim3 grid((unsigned)((n_pole + 255) / 256), (unsigned)(row_blocks + 1));
+  if (aligned16(xi, ldxi) && aligned16(Z, ldz))
+    casida_z_kernel<2><<<grid, 128, 0, stream>>>(eps, n_mo, n_occ, lambda, xi, ldxi, n_pole, Omega, Z, ldz);
+  else
+    casida_z_kernel<1><<<grid, 128, 0, stream>>>(eps, n_mo, n_occ, lambda, xi, ldxi, n_pole, Omega, Z, ldz);
+  QSGW_CUDA(nullptr, cudaGetLastError());
   return QSGW_SIGMA_OK;
 }
 

@@ -104,6 +104,77 @@ __global__ void check_range_kernel(const double *__restrict__ x, int64_t n, doub
   if (bad) atomicAdd(out, bad);
 }
 
+// ---------------------------------------------------------------- Casida / RPA step (row 8(f).4)
+// Bov[P][ia] = B[P][i][a] (k-major operand of the C-matrix GEMM; ia = i*v + (a-o)), and for blockIdx.y == n_aux:
+// d[ia] = Delta_ia = eps[a] - eps[i], sqd[ia] = sqrt(Delta_ia).
+__global__ void casida_gather_kernel(const double *__restrict__ B, const double *__restrict__ eps, int n_mo, int n_occ, int n_aux,
+                                     double *__restrict__ Bov, int64_t ld_ov, double *__restrict__ d, double *__restrict__ sqd) {
+  const int v = n_mo - n_occ;
+  const int64_t n_ov = (int64_t)n_occ * v;
+  const int64_t ia = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (ia >= n_ov) return;
+  const int i = (int)(ia / v), a = n_occ + (int)(ia - (int64_t)i * v);
+  const int P = blockIdx.y;
+  if (P < n_aux) {
+    Bov[(int64_t)P * ld_ov + ia] = B[((int64_t)P * n_mo + i) * n_mo + a];
+  } else {
+    const double dd = eps[a] - eps[i];
+    d[ia] = dd;
+    sqd[ia] = sqrt(dd);
+  }
+}
+
+// blockIdx.y == gridDim.y - 1 (one extra row of blocks): Omega[s] = sqrt(lambda[s]);
+// otherwise Z[ia][s] = sqrt(Delta_ia) * xi[ia][s] / sqrt(Omega_s) for the rows ia = blockIdx.y * 8 .. + 7  (X + Y of Eq. (18)).
+// HBM-bound (xi read once, Z written once): a thread owns two adjacent poles and issues the loads of its 8 rows before it
+// uses any of them; VEC = 2 needs xi and Z 16-byte aligned with even leading dimensions.
+template <int VEC>
+__global__ void __launch_bounds__(128)
+casida_z_kernel(const double *__restrict__ eps, int n_mo, int n_occ, const double *__restrict__ lambda,
+                const double *__restrict__ xi, int64_t ldxi, int64_t n_pole, double *__restrict__ Omega,
+                double *__restrict__ Z, int64_t ldz) {
+  const int64_t s = 2 * (blockIdx.x * (int64_t)blockDim.x + threadIdx.x);
+  if (s >= n_pole) return;
+  const bool two = s + 1 < n_pole;
+  const double om0 = sqrt(__ldg(lambda + s)), om1 = two ? sqrt(__ldg(lambda + s + 1)) : 1.0;
+  if (blockIdx.y == gridDim.y - 1) {
+    Omega[s] = om0;
+    if (two) Omega[s + 1] = om1;
+    return;
+  }
+  const double rs0 = 1.0 / sqrt(om0), rs1 = 1.0 / sqrt(om1);
+  const int v = n_mo - n_occ;
+  const int64_t n_ov = (int64_t)n_occ * v;
+  const int64_t ia0 = (int64_t)blockIdx.y * 8;
+  double x0[8], x1[8], sd[8];
+#pragma unroll
+  for (int r = 0; r < 8; ++r) {
+    const int64_t ia = min(ia0 + r, n_ov - 1);
+    const int i = (int)(ia / v), a = n_occ + (int)(ia - (int64_t)i * v);
+    sd[r] = sqrt(__ldg(eps + a) - __ldg(eps + i));
+    if (VEC == 2 && two) {
+      const double2 t = *reinterpret_cast<const double2 *>(xi + ia * ldxi + s);
+      x0[r] = t.x; x1[r] = t.y;
+    } else {
+      x0[r] = xi[ia * ldxi + s];
+      x1[r] = two ? xi[ia * ldxi + s + 1] : 0.0;
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < 8; ++r) {
+    const int64_t ia = ia0 + r;
+    if (ia < n_ov) {
+      const double z0 = sd[r] * x0[r] * rs0, z1 = sd[r] * x1[r] * rs1;
+      if (VEC == 2 && two) {
+        *reinterpret_cast<double2 *>(Z + ia * ldz + s) = make_double2(z0, z1);
+      } else {
+        Z[ia * ldz + s] = z0;
+        if (two) Z[ia * ldz + s + 1] = z1;
+      }
+    }
+  }
+}
+
 // ---------------------------------------------------------------- epilogue
 // T = sum_z Tpart[z] in a fixed order, then Eq. (19): Sigma[p][q] = Sigma[q][p] = (T[p][q]+T[q][p])/2, both written
 // from the same expression so the output is bit-symmetric.  grid = (nt, nt) tiles of 16 x 16, blocks below the
