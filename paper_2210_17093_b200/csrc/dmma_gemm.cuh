@@ -119,6 +119,26 @@ __device__ __forceinline__ void mma_ktile_kmajor_frag(double (&acc)[8][4][2], co
   }
 }
 
+// A full tile's LAST k-tile when K is not a multiple of the ring depth: only the first nsteps k4 steps hold rows k < K (the
+// producers zero-filled the rest), so the others are skipped instead of multiplied (K = 1100: 12 of the last 32 rows).
+__device__ __forceinline__ void mma_ktile_kmajor_partial(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm,
+                                                         int nsteps) {
+  const double *ap = as + 8 * fm.wmi + fm.g + fm.t * kLdT;
+  const double *bp = bs + 8 * fm.wni + fm.g + fm.t * kLdT;
+#pragma unroll 1
+  for (int kk = 0; kk < nsteps; ++kk) {
+    double a[8], b[4];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = ap[kk * 4 * kLdT + 16 * i];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) b[j] = bp[kk * 4 * kLdT + 32 * j];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) dmma_m8n8k4(acc[i][j], a[i], b[j]);
+  }
+}
+
 template <int NJ>
 __device__ __forceinline__ void mma_ktile_kmajor_mi(double (&acc)[8][4][2], const double *as, const double *bs, const FragMap &fm) {
   switch (fm.mi_cnt) {
@@ -342,7 +362,9 @@ gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__
       decode_tile(t, ntm, ntn, m_fastest, tri, tm, tn);
       const int m0 = tm * kBM, n0 = tn * kBN;
       const Epi epi = epi0.for_batch(batch);
-      const int KT = (batch_depth(K, k_total, batch) + kGBK - 1) / kGBK;
+      const int Kb = batch_depth(K, k_total, batch);
+      const int KT = (Kb + kGBK - 1) / kGBK;
+      const int last_steps = (Kb - (KT - 1) * kGBK + 3) >> 2;       // k4 steps of the last k-tile that hold rows k < K
       const FragMap fm(warp, lane, M - m0, N - n0);
       const bool full_tile = fm.mi_cnt == 8 && fm.nj_cnt == 4;
       // per-row epilogue context (stage 2: the (p, m) pair of the row), fetched now so its latency hides behind the k loop
@@ -357,7 +379,9 @@ gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__
 #pragma unroll 1
       for (int kt = 0; kt < KT; ++kt) {
         mbar_wait(full + st, ph);
-        if (full_tile) mma_ktile_kmajor_frag<8, 4>(acc, As + st * kGBK * kLdT, Bs + st * kGBK * kLdT, fm);
+        if (full_tile && kt == KT - 1 && last_steps < kGBK / 4)
+          mma_ktile_kmajor_partial(acc, As + st * kGBK * kLdT, Bs + st * kGBK * kLdT, fm, last_steps);
+        else if (full_tile) mma_ktile_kmajor_frag<8, 4>(acc, As + st * kGBK * kLdT, Bs + st * kGBK * kLdT, fm);
         else mma_ktile_kmajor_any(acc, As + st * kGBK * kLdT, Bs + st * kGBK * kLdT, fm);
         __syncwarp();
         if (lane == 0) mbar_arrive(empty + st);

@@ -11,11 +11,12 @@
 //     swizzle, out-of-range rows / poles zero-filled by the hardware), issued by ONE elected thread;
 //   * k-tiles are 32 poles deep at one m (two 16-pole = 128-byte halves), so eps_m / f_m are CTA-uniform per k-tile;
 //   * the two operands have their own rings: the p rows (16 KB per k-tile) sit in a DEEP ring, because they must be
-//     scaled by D before use -- the four producer warps multiply them in place, several k-tiles ahead of the DMMA
+//     scaled by D before use -- three producer warps multiply them in place, several k-tiles ahead of the DMMA
 //     warps, so that the latency of their FP64 bursts (they share the FP64 pipe with the DMMAs and are served in its
-//     gaps) stays off the critical path; the q rows (up to 64 KB per k-tile) go straight from TMA to the DMMA warps
-//     through a shallow ring;
-//   * 8 consumer warps (2 x 4) run LDS.64 fragment loads + DMMA.8x8x4 only; accumulators in registers;
+//     gaps) stays off the critical path; the q rows go straight from TMA to the DMMA warps through a ring managed in
+//     16-pole halves of a k-tile (a half is released, and its refill issued, as soon as it has been consumed);
+//   * 8 consumer warps (2 x 4) run LDS.64 fragment loads + DMMA.8x8x4 only, software-pipelined across k4 steps and ring
+//     stages (the next fragments, barrier waits included, are fetched under the current DMMAs); accumulators in registers;
 //   * split-K over m into slot-owned partial tiles (fixed accumulation order, no atomics).
 #pragma once
 #include <cuda.h>
@@ -51,28 +52,28 @@ constexpr int kHalfRowBytes = 128;
 constexpr int kAStageBytes = 2 * kTP * kHalfRowBytes;   // 16 KB
 constexpr int kMaxAStages = 6;
 constexpr int kScaleWarps = 3;           // producer warps that scale (the fourth issues the TMA loads)
-constexpr int kMaxBStages = 4;
+constexpr int kMaxBStages = 8;           // q-row ring stages (each ONE 16-pole half of a k-tile)
 constexpr size_t kSigmaSmemBudget = 227 * 1024 - 1024;  // dynamic shared memory of one CTA, less the alignment slack
 
 struct SigmaRings {
-  int nA, nB;            // ring depths
-  int b_stage_bytes;     // 2 * tq * 128
+  int nA, nB;            // ring depths: p ring in k-tiles, q ring in 16-pole HALVES of a k-tile
+  int b_stage_bytes;     // tq * 128: one half of a k-tile of q rows
   size_t smem_bytes;     // dynamic shared memory to launch with (includes 1 KB of alignment slack and the barriers)
 };
 
-// Ring depths for a tile tq columns wide.  The p ring gets 6 stages if the q ring still has 2 (one being read, three
-// being scaled by the three scaling warps, two landing); the q ring takes the stages that fit beside them (at most 4).
-// Measured at N = 600: a third q stage at the expense of two p stages is slower (583 vs 578 ms per build).
+// Ring depths for a tile tq columns wide.  The q rows go straight from TMA to the DMMA warps, so their ring is what hides
+// the load latency: it is managed in half k-tiles (a stage is released -- and its refill issued -- as soon as its 16 poles
+// are consumed) and gets the shared memory the p ring does not need.  The p ring keeps nA k-tiles: one being read, up to
+// three being scaled by the three scaling warps, the rest landing.
 inline SigmaRings sigma_rings(int tq) {
   SigmaRings r;
-  r.b_stage_bytes = 2 * tq * kHalfRowBytes;
+  r.b_stage_bytes = tq * kHalfRowBytes;
   const size_t bar_bytes = 1024;
   const size_t avail = kSigmaSmemBudget - bar_bytes;
-  r.nB = (int)((avail - 6 * (size_t)kAStageBytes) / r.b_stage_bytes);
+  r.nA = 6;
+  r.nB = (int)((avail - (size_t)r.nA * kAStageBytes) / r.b_stage_bytes);
   if (r.nB > kMaxBStages) r.nB = kMaxBStages;
   if (r.nB < 2) r.nB = 2;
-  r.nA = (int)((avail - (size_t)r.nB * r.b_stage_bytes) / kAStageBytes);
-  if (r.nA > kMaxAStages) r.nA = kMaxAStages;
   r.smem_bytes = 1024 + (size_t)r.nA * kAStageBytes + (size_t)r.nB * r.b_stage_bytes + bar_bytes;
   return r;
 }
@@ -116,61 +117,157 @@ struct SigmaFragMap {
   __device__ __forceinline__ int out_col(int j) const { return 32 * j + 8 * wni + 2 * t; }
 };
 
-// One 16-pole half of a k-tile: acc[i][j] += A[p rows of fragment i][k] * Wq[q rows of fragment j][k], k = 0..15, for
-// the first MI x NJ fragments of the warp.  ap / bp: this lane's row (8 wmi + g resp. 8 wni + g) of the half, at byte
-// offset 8 (t & 1); sw[kk]: the lane's swizzled 16-byte chunk offset of k4 step kk.  Rows are 128 bytes; fragment i of
-// the p operand is 16 rows further, fragment j of the q operand 32 rows.  MI, NJ are compile-time: a predicated-off
-// DMMA still occupies the FP64 pipe for its full issue time, so ragged edge tiles BRANCH around unowned fragments.
+// Ring state of the DMMA warps, as 32-bit shared-window addresses (few registers: the accumulators take 128 of them).
+struct SigmaConsumerRings {
+  uint32_t a_ring, b_ring;            // ring bases plus this lane's row / byte offset
+  uint32_t a_full, a_empty, b_full, b_empty;   // barrier arrays (8 bytes per stage)
+  int nA, nB, b_stage_bytes;
+};
+
+__device__ __forceinline__ double lds_f64(uint32_t addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void mbar_wait_s(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_s(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
+// The whole k loop of a CTA tile for the first MI x NJ fragments of the warp: acc[i][j] += A[p rows of fragment i][k] *
+// Wq[q rows of fragment j][k] over the KT k-tiles of the split-K slot, two 16-pole halves per k-tile, four k4 steps per
+// half.  Rows are 128 bytes; fragment i of the p operand is 16 rows further, fragment j of the q operand 32 rows; sw[kk]
+// is the lane's swizzled 16-byte chunk offset of k4 step kk.  MI, NJ are compile-time: a predicated-off DMMA still
+// occupies the FP64 pipe for its full issue time, so ragged edge tiles BRANCH around unowned fragments.
+// Software-pipelined across k4 steps AND ring stages without a second set of fragment registers: the fragments of the
+// next step are fetched into the registers of this step as they fall free (a[i] after the DMMAs of row i, b[j] during
+// the last row); at the last step of a half the barrier waits of the next half come first.  The q-row stage of a half
+// is released as soon as that half is consumed; the p-row stage after both halves.
 template <int MI, int NJ>
-__device__ __forceinline__ void mma_half_sigma(double (&acc)[4][8][2], const char *ap, const char *bp, const int (&sw)[4]) {
+__device__ __forceinline__ void sigma_consumer_kloop(double (&acc)[4][8][2], const SigmaConsumerRings &r, uint32_t sw0, int KT, int lane) {
+  int sa = 0, sb = 0;
+  uint32_t pha = 0, phb = 0;
+  double a[MI], b[NJ];
+  mbar_wait_s(r.b_full, 0);
+  mbar_wait_s(r.a_full, 0);
+  uint32_t ap = r.a_ring, bp = r.b_ring;
 #pragma unroll
-  for (int kk = 0; kk < 4; ++kk) {
-    double a[MI], b[NJ];
+  for (int i = 0; i < MI; ++i) a[i] = lds_f64((ap ^ sw0) + 16 * i * kHalfRowBytes);
 #pragma unroll
-    for (int i = 0; i < MI; ++i) a[i] = *reinterpret_cast<const double *>(ap + 16 * i * kHalfRowBytes + sw[kk]);
+  for (int j = 0; j < NJ; ++j) b[j] = lds_f64((bp ^ sw0) + 32 * j * kHalfRowBytes);
+#pragma unroll 1
+  for (int kt = 0; kt < KT; ++kt) {
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) b[j] = *reinterpret_cast<const double *>(bp + 32 * j * kHalfRowBytes + sw[kk]);
+    for (int h = 0; h < 2; ++h) {
 #pragma unroll
-    for (int i = 0; i < MI; ++i)
+      for (int kk = 0; kk < 4; ++kk) {
+        // sw[kk] = sw0 ^ (kk << 4), applied with XOR: the lane offsets in ap / bp are multiples of 128 plus 0 or 8, so
+        // bits 4..6 of the address are free
+        const bool edge = (kk == 3);
+        bool fetch = true;
+        uint32_t apx, bpx;
+        if (edge) {
+          fetch = (h == 0) || (kt + 1 < KT);
+          const int sb_n = (sb + 1 == r.nB) ? 0 : sb + 1;
+          const int sa_n = h ? ((sa + 1 == r.nA) ? 0 : sa + 1) : sa;
+          if (fetch) {
+            mbar_wait_s(r.b_full + 8 * sb_n, (sb + 1 == r.nB) ? phb ^ 1 : phb);
+            if (h) mbar_wait_s(r.a_full + 8 * sa_n, (sa + 1 == r.nA) ? pha ^ 1 : pha);
+          }
+          apx = (r.a_ring + sa_n * kAStageBytes + (h ? 0 : kTP * kHalfRowBytes));
+          bpx = (r.b_ring + sb_n * r.b_stage_bytes);
+        } else {
+          apx = ap ^ ((kk + 1) << 4);
+          bpx = bp ^ ((kk + 1) << 4);
+        }
+        apx ^= sw0;
+        bpx ^= sw0;
 #pragma unroll
-      for (int j = 0; j < NJ; ++j) dmma_m8n8k4(acc[i][j], a[i], b[j]);
+        for (int i = 0; i < MI; ++i) {
+#pragma unroll
+          for (int j = 0; j < NJ; ++j) {
+            dmma_m8n8k4(acc[i][j], a[i], b[j]);
+            if (i == MI - 1 && fetch) b[j] = lds_f64(bpx + 32 * j * kHalfRowBytes);
+          }
+          if (fetch) a[i] = lds_f64(apx + 16 * i * kHalfRowBytes);
+        }
+      }
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive_s(r.b_empty + 8 * sb);         // this half of the q rows can be refilled while the other is in use
+        if (h) mbar_arrive_s(r.a_empty + 8 * sa);
+      }
+      if (++sb == r.nB) { sb = 0; phb ^= 1; }
+      if (h && ++sa == r.nA) { sa = 0; pha ^= 1; }
+      ap = r.a_ring + sa * kAStageBytes + (h ? 0 : kTP * kHalfRowBytes);
+      bp = r.b_ring + sb * r.b_stage_bytes;
+    }
   }
 }
 
 template <int MI>
-__device__ __forceinline__ void mma_half_sigma_nj(double (&acc)[4][8][2], const char *ap, const char *bp, const int (&sw)[4], int nj) {
+__device__ __forceinline__ void sigma_consumer_kloop_nj(double (&acc)[4][8][2], const SigmaConsumerRings &r, uint32_t sw, int KT,
+                                                        int lane, int nj) {
   switch (nj) {
-    case 1: mma_half_sigma<MI, 1>(acc, ap, bp, sw); break;
-    case 2: mma_half_sigma<MI, 2>(acc, ap, bp, sw); break;
-    case 3: mma_half_sigma<MI, 3>(acc, ap, bp, sw); break;
-    case 4: mma_half_sigma<MI, 4>(acc, ap, bp, sw); break;
-    case 5: mma_half_sigma<MI, 5>(acc, ap, bp, sw); break;
-    case 6: mma_half_sigma<MI, 6>(acc, ap, bp, sw); break;
-    case 7: mma_half_sigma<MI, 7>(acc, ap, bp, sw); break;
-    case 8: mma_half_sigma<MI, 8>(acc, ap, bp, sw); break;
-    default: break;
+    case 1: sigma_consumer_kloop<MI, 1>(acc, r, sw, KT, lane); break;
+    case 2: sigma_consumer_kloop<MI, 2>(acc, r, sw, KT, lane); break;
+    case 3: sigma_consumer_kloop<MI, 3>(acc, r, sw, KT, lane); break;
+    case 4: sigma_consumer_kloop<MI, 4>(acc, r, sw, KT, lane); break;
+    case 5: sigma_consumer_kloop<MI, 5>(acc, r, sw, KT, lane); break;
+    case 6: sigma_consumer_kloop<MI, 6>(acc, r, sw, KT, lane); break;
+    case 7: sigma_consumer_kloop<MI, 7>(acc, r, sw, KT, lane); break;
+    default: sigma_consumer_kloop<MI, 8>(acc, r, sw, KT, lane); break;
   }
 }
 
-// Ragged tile: dispatch (warp-uniform) on the fragment counts of this warp.
-__device__ __forceinline__ void mma_half_sigma_ragged(double (&acc)[4][8][2], const char *ap, const char *bp, const int (&sw)[4],
-                                                      int mi, int nj) {
+// Ragged tile: dispatch (warp-uniform) on the fragment counts of this warp.  A warp without any fragment still walks the
+// rings: it owes the issuer its `empty` arrivals.
+__device__ __forceinline__ void sigma_consumer_kloop_ragged(double (&acc)[4][8][2], const SigmaConsumerRings &r, uint32_t sw,
+                                                            int KT, int lane, int mi, int nj) {
+  if (mi == 0 || nj == 0) {
+    int sa = 0, sb = 0;
+    uint32_t pha = 0, phb = 0;
+#pragma unroll 1
+    for (int kt = 0; kt < KT; ++kt) {
+      mbar_wait_s(r.a_full + 8 * sa, pha);
+      for (int h = 0; h < 2; ++h) {
+        mbar_wait_s(r.b_full + 8 * sb, phb);
+        __syncwarp();
+        if (lane == 0) mbar_arrive_s(r.b_empty + 8 * sb);
+        if (++sb == r.nB) { sb = 0; phb ^= 1; }
+      }
+      if (lane == 0) mbar_arrive_s(r.a_empty + 8 * sa);
+      if (++sa == r.nA) { sa = 0; pha ^= 1; }
+    }
+    return;
+  }
   switch (mi) {
-    case 1: mma_half_sigma_nj<1>(acc, ap, bp, sw, nj); break;
-    case 2: mma_half_sigma_nj<2>(acc, ap, bp, sw, nj); break;
-    case 3: mma_half_sigma_nj<3>(acc, ap, bp, sw, nj); break;
-    case 4: mma_half_sigma_nj<4>(acc, ap, bp, sw, nj); break;
-    default: break;
+    case 1: sigma_consumer_kloop_nj<1>(acc, r, sw, KT, lane, nj); break;
+    case 2: sigma_consumer_kloop_nj<2>(acc, r, sw, KT, lane, nj); break;
+    case 3: sigma_consumer_kloop_nj<3>(acc, r, sw, KT, lane, nj); break;
+    default: sigma_consumer_kloop_nj<4>(acc, r, sw, KT, lane, nj); break;
   }
 }
 
-// One CTA: output tile (tp, tq) of T, 64 x tq, for the k-tiles of split-K slot z = blockIdx.y: a contiguous range of the
+// One CTA: output tile (tp, tq) of T, 64 x tq, for the k-tiles of split-K slot z: a contiguous range of the
 // (m, 32-pole group) pairs of the chunk (s_c poles, all internal states m).
 //   mapA  tensor map of the left operand (scaled by D)  [m][p][s], box {16 poles, 64 rows, 1}.  qsGW: the w chunk of
 //         stage 2 (both mirrors present); qsMP2 exchange term: the exchange integrals (pi|an)
 //   mapB  tensor map of the right operand, same indexing, box {16 poles, tq rows, 1}.  qsGW: the same array
 //   Omega [s_c]  excitation energies of the chunk
-//   Tpart [nsplit][N][N]  split-K partial tiles; slot z is owned by the CTAs with blockIdx.y == z and is
+//   Tpart [nsplit][N][N]  split-K partial tiles; slot z is owned by the CTAs of that slot and is
 //         read-modify-written once per launch -> accumulation order is fixed, results reproducible.
 __global__ void __launch_bounds__(kThreads, 1)
 sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
@@ -181,7 +278,7 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
   // the 128-byte swizzle pattern is a function of the shared-memory ADDRESS: stage bases must be 1024-byte aligned
   // (offset added to the __shared__ array itself, so that the compiler keeps emitting LDS / STS rather than generic accesses)
   uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-  const int b_stage_bytes = 2 * tq * kHalfRowBytes;
+  const int b_stage_bytes = tq * kHalfRowBytes;   // one 16-pole half of a k-tile
   uint8_t *a_ring = smem;
   uint8_t *b_ring = smem + nA * kAStageBytes;
   uint64_t *bars = reinterpret_cast<uint64_t *>(b_ring + (size_t)nB * b_stage_bytes);
@@ -192,12 +289,23 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
   uint64_t *b_empty = b_full + kMaxBStages;     // [nB] read by all consumer warps       -> TMA issuer
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tp = blockIdx.x / ntq, tqi = blockIdx.x - tp * ntq;
+  // CTA -> (tile, split-K slot z).  CTAs start in the order of their linear index; the tiles of the last, short p row
+  // (N mod 64 rows) run 2-3 times shorter than the others, so they are numbered LAST: the end of the launch is filled
+  // with short CTAs instead of waiting for a long one.  Within either group the tile index varies fastest, so the CTAs
+  // of one slot (same m range, same w rows) run at the same time and share those rows in L2.
+  int tile, z;
+  {
+    const int ntiles = gridDim.x, nfull = (n_mo / kTP) * ntq, nrag = ntiles - nfull;
+    const int lin = blockIdx.y * ntiles + blockIdx.x;
+    if (lin < nfull * nsplit) { z = lin / nfull; tile = lin - z * nfull; }
+    else { const int l2 = lin - nfull * nsplit; z = l2 / nrag; tile = nfull + (l2 - z * nrag); }
+  }
+  const int tp = tile / ntq, tqi = tile - tp * ntq;
   const int p0 = tp * kTP, q0 = tqi * tq;
   // split-K: the k-tiles (m, ks), numbered m * KTS + ks, are dealt to the nsplit slots in equal contiguous ranges
   const int KTS = (s_c + kKD - 1) / kKD;         // k-tiles per m
-  const int kt_begin = (int)((int64_t)n_mo * KTS * blockIdx.y / nsplit);
-  const int KT = (int)((int64_t)n_mo * KTS * (blockIdx.y + 1) / nsplit) - kt_begin;
+  const int kt_begin = (int)((int64_t)n_mo * KTS * z / nsplit);
+  const int KT = (int)((int64_t)n_mo * KTS * (z + 1) / nsplit) - kt_begin;
 
   if (tid == 0) {
     for (int s = 0; s < nA; ++s) {
@@ -213,6 +321,7 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
   }
   __syncthreads();
 
+  // registers are a per-sub-partition resource (16 K each, holding two DMMA warps and one producer warp): 2 x 184 + 136
   if (warp >= kConsumerWarps) reg_dec<136>();     // the whole producer warpgroup, one instruction
   if (warp == kConsumerWarps) {
     // ------------------------------------------------ TMA issuer (one elected thread of the first producer warp)
@@ -221,10 +330,11 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
     if (lane == 0) {
       int a_next = 0, a_st = 0, a_m = kt_begin / KTS, a_ks = kt_begin - (kt_begin / KTS) * KTS;
       uint32_t a_ph = 1;                          // a fresh barrier passes a wait on parity 1
-      int b_next = 0, b_st = 0, b_m = a_m, b_ks = a_ks;
+      int b_next = 0, b_st = 0, b_m = a_m, b_s0 = a_ks * kKD;     // the q ring advances in halves of a k-tile
       uint32_t b_ph = 1;
+      const int KTB = 2 * KT, s_end = KTS * kKD;
       // both rings in k-tile order, never blocking on one ring while the other has a free stage
-      while (a_next < KT || b_next < KT) {
+      while (a_next < KT || b_next < KTB) {
         bool issued = false;
         if (a_next < KT && mbar_test(a_empty + a_st, a_ph)) {
           mbar_arrive_expect_tx(a_raw + a_st, kAStageBytes);
@@ -236,13 +346,11 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
           if (++a_st == nA) { a_st = 0; a_ph ^= 1; }
           issued = true;
         }
-        if (b_next < KT && mbar_test(b_empty + b_st, b_ph)) {
+        if (b_next < KTB && mbar_test(b_empty + b_st, b_ph)) {
           mbar_arrive_expect_tx(b_full + b_st, b_stage_bytes);
-          const uint32_t dst = smem_u32(b_ring + (size_t)b_st * b_stage_bytes);
-          tma_load_3d(dst, &mapB, b_full + b_st, b_ks * kKD, q0, b_m);
-          tma_load_3d(dst + tq * kHalfRowBytes, &mapB, b_full + b_st, b_ks * kKD + 16, q0, b_m);
+          tma_load_3d(smem_u32(b_ring + (size_t)b_st * b_stage_bytes), &mapB, b_full + b_st, b_s0, q0, b_m);
           ++b_next;
-          if (++b_ks == KTS) { b_ks = 0; ++b_m; }
+          if ((b_s0 += 16) == s_end) { b_s0 = 0; ++b_m; }
           if (++b_st == nB) { b_st = 0; b_ph ^= 1; }
           issued = true;
         }
@@ -348,36 +456,21 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
     // (the contraction sums over all of them), so lane t of step kk takes pole 8 (t >> 1) + 2 kk + (t & 1): chunk
     // 4 (t >> 1) + kk, half (t & 1) of it.  The 16 lanes of a half warp (4 rows g x 4 t) then hit 16 distinct 8-byte
     // bank pairs -- with the natural choice 4 kk + t, rows g and g ^ 1 would collide on the same two chunks.
-    int sw[4];
-#pragma unroll
-    for (int kk = 0; kk < 4; ++kk) sw[kk] = (kk ^ (fm.g ^ ((fm.t >> 1) << 2))) << 4;
+    const uint32_t sw = (uint32_t)(fm.g ^ ((fm.t >> 1) << 2)) << 4;   // k4 step kk reads chunk offset sw ^ (kk << 4)
     const int a_lane = (8 * fm.wmi + fm.g) * kHalfRowBytes + 8 * (fm.t & 1);
     const int b_lane = (8 * fm.wni + fm.g) * kHalfRowBytes + 8 * (fm.t & 1);
-    int sa = 0, sb = 0;
-    uint32_t pha = 0, phb = 0;
-#pragma unroll 1
-    for (int kt = 0; kt < KT; ++kt) {
-      mbar_wait(b_full + sb, phb);
-      mbar_wait(a_full + sa, pha);
-      const char *ap = reinterpret_cast<const char *>(a_ring + sa * kAStageBytes) + a_lane;
-      const char *bp = reinterpret_cast<const char *>(b_ring + (size_t)sb * b_stage_bytes) + b_lane;
-      if (full_tile) {
-        mma_half_sigma<4, 8>(acc, ap, bp, sw);
-        mma_half_sigma<4, 8>(acc, ap + kTP * kHalfRowBytes, bp + tq * kHalfRowBytes, sw);
-      } else {
-        mma_half_sigma_ragged(acc, ap, bp, sw, fm.mi_cnt, fm.nj_cnt);
-        mma_half_sigma_ragged(acc, ap + kTP * kHalfRowBytes, bp + tq * kHalfRowBytes, sw, fm.mi_cnt, fm.nj_cnt);
-      }
-      __syncwarp();
-      if (lane == 0) {
-        mbar_arrive(a_empty + sa);
-        mbar_arrive(b_empty + sb);
-      }
-      if (++sa == nA) { sa = 0; pha ^= 1; }
-      if (++sb == nB) { sb = 0; phb ^= 1; }
+    SigmaConsumerRings rings;
+    rings.a_ring = smem_u32(a_ring) + a_lane;
+    rings.b_ring = smem_u32(b_ring) + b_lane;
+    rings.a_full = smem_u32(a_full); rings.a_empty = smem_u32(a_empty);
+    rings.b_full = smem_u32(b_full); rings.b_empty = smem_u32(b_empty);
+    rings.nA = nA; rings.nB = nB; rings.b_stage_bytes = b_stage_bytes;
+    if (KT > 0) {
+      if (full_tile) sigma_consumer_kloop<4, 8>(acc, rings, sw, KT, lane);
+      else sigma_consumer_kloop_ragged(acc, rings, sw, KT, lane, fm.mi_cnt, fm.nj_cnt);
     }
 
-    double *Tz = Tpart + (int64_t)blockIdx.y * n_mo * n_mo;
+    double *Tz = Tpart + (int64_t)z * n_mo * n_mo;
     const bool vec_ok = (n_mo & 1) == 0;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
