@@ -131,6 +131,8 @@ int qsgw_sigma_finish(qsgw_sigma_plan *plan, double *Sigma);
  * next range with the kernels of the current one, downloads Sigma and synchronises before returning.
  * n_pole may exceed n_pole_max.  Device staging buffers for the host path are allocated on the first
  * call (not in create) and kept by the plan; ALLOC if they do not fit.
+ * Of B only the entries B[P][p][q] with p <= q are read (and uploaded): B is symmetric in its last two
+ * indices (precondition), and the build uses nothing else.  In debug mode all of B is uploaded and checked.
  */
 int qsgw_sigma_build_host(qsgw_sigma_plan *plan, const double *B, const double *eps, const double *occ,
                           const double *Omega, const double *Z, int64_t ldz, int64_t n_pole, double eta,

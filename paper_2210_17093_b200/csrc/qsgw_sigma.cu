@@ -802,8 +802,25 @@ int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps
   const int64_t R = p->h_range, ldr = round_up(R, 2);
   const size_t nn = (size_t)p->n_mo * p->n_mo;
 
-  // B, eps, occ on the compute stream (begin needs them first)
-  QSGW_CUDA(p, cudaMemcpyAsync(p->hB, B, sizeof(double) * p->n_aux * nn, cudaMemcpyHostToDevice, p->stream));
+  // B, eps, occ on the compute stream (begin needs them first).  The build reads B[P][p][q] only for p <= q (B is symmetric
+  // in its last two indices: the pair pack takes p <= m, the stage-1 block i < o <= a), so only that part is uploaded:
+  // row blocks [r0, r1) x columns [r0, N) for all P, one strided 3-D copy each -- 54 % of the bytes of B with 12 blocks.
+  // Debug mode checks the symmetry of B on the device and therefore uploads all of it.
+  if (p->debug) {
+    QSGW_CUDA(p, cudaMemcpyAsync(p->hB, B, sizeof(double) * p->n_aux * nn, cudaMemcpyHostToDevice, p->stream));
+  } else {
+    const int N = p->n_mo, nblk = std::min(12, std::max(1, N / 32));
+    for (int b = 0; b < nblk; ++b) {
+      const int r0 = (int)((int64_t)N * b / nblk), r1 = (int)((int64_t)N * (b + 1) / nblk);
+      cudaMemcpy3DParms cp = {};
+      const size_t off = (size_t)r0 * N + r0;
+      cp.srcPtr = make_cudaPitchedPtr(const_cast<double *>(B) + off, sizeof(double) * N, N, N);
+      cp.dstPtr = make_cudaPitchedPtr(p->hB + off, sizeof(double) * N, N, N);
+      cp.extent = make_cudaExtent(sizeof(double) * (size_t)(N - r0), (size_t)(r1 - r0), (size_t)p->n_aux);
+      cp.kind = cudaMemcpyHostToDevice;
+      QSGW_CUDA(p, cudaMemcpy3DAsync(&cp, p->stream));
+    }
+  }
   QSGW_CUDA(p, cudaMemcpyAsync(p->hEps, eps, sizeof(double) * p->n_mo, cudaMemcpyHostToDevice, p->stream));
   QSGW_CUDA(p, cudaMemcpyAsync(p->hOcc, occ, sizeof(double) * p->n_mo, cudaMemcpyHostToDevice, p->stream));
 
