@@ -202,6 +202,43 @@ __device__ __forceinline__ void load_tile_kmajor(double *dst, const double *src,
   }
 }
 
+// ---- bulk-copy producer (both operands 16-byte aligned with even leading dimensions)
+// One k-row of an operand tile is 128 contiguous doubles in global memory and one padded row of the shared tile, so it
+// travels as ONE cp.async.bulk (1 KB, the TMA unit's linear copy, completion counted in bytes on the stage's mbarrier)
+// issued by the lane that owns the row: warp 0 of the producers moves the 32 rows of A, warp 1 those of B.  Against
+// 16-byte LDGSTS copies through the LSU / L1 path this removes the producers' data return from the path of the DMMA
+// warps' fragment loads (measured at the `large` config: the LDGSTS producers cost stage 2 2.3 %).
+// Ragged tiles copy round_up(cvalid, 2) columns (the source row has an even leading dimension, so the extra column is
+// inside it; columns >= cvalid only reach output columns that are not stored).  Rows k >= kvalid of a last k-tile are
+// zero-filled by their lane with ordinary stores.
+__device__ __forceinline__ void bulk_copy_row(uint32_t smem_dst, const double *src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_dst), "l"(src),
+               "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx_u32(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// Lane `lane` (= k-row of the tile) of one producer warp: dst = shared tile [kGBK][kLdT], src = first valid element of the
+// tile (row 0), ld its leading dimension.
+__device__ __forceinline__ void bulk_load_tile_kmajor(double *dst, const double *src, int64_t ld, int kvalid, int cvalid, uint64_t *bar,
+                                                      int lane) {
+  const int cols = min(kBM, (max(cvalid, 0) + 1) & ~1);
+  const int rows = min(kvalid, kGBK);
+  const uint32_t bar32 = smem_u32(bar);
+  if (lane == 0) mbar_arrive_expect_tx_u32(bar32, (uint32_t)(rows * cols * (int)sizeof(double)));
+  __syncwarp();
+  if (lane < rows) {
+    bulk_copy_row(smem_u32(dst + lane * kLdT), src + (int64_t)lane * ld, (uint32_t)(cols * (int)sizeof(double)), bar32);
+  } else {
+    double2 *row = reinterpret_cast<double2 *>(dst + lane * kLdT);
+#pragma unroll 4
+    for (int c = 0; c < kBM / 2; ++c) row[c] = make_double2(0.0, 0.0);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // a later bulk copy (async proxy) reuses these rows
+  }
+  if (lane != 0) mbar_arrive(bar);
+}
+
 // ---------------------------------------------------------------- epilogues
 // C[row][col] = alpha * acc   (stage 1: V, alpha = 1; AO->MO half transforms); batch b writes at C + b * strideC.
 struct EpiStore {
@@ -317,7 +354,7 @@ gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__
 
   if (tid == 0) {
     for (int s = 0; s < kGemmStages; ++s) {
-      mbar_init(full + s, kProducerThreads);
+      mbar_init(full + s, (VECA == 2 && VECB == 2) ? 64 : kProducerThreads);   // bulk producers: the lanes of two warps
       mbar_init(empty + s, kConsumerWarps);
     }
     mbar_fence_init();
@@ -342,11 +379,20 @@ gemm_tn_dmma_kernel(const double *__restrict__ A0, int64_t lda, const double *__
       const int Kb = batch_depth(K, k_total, batch);
       const int KT = (Kb + kGBK - 1) / kGBK;
       for (int kt = 0; kt < KT; ++kt) {
-        mbar_wait(empty + st, ph);
         const int k0 = kt * kGBK;
-        load_tile_kmajor<VECA>(As + st * kGBK * kLdT, A + (int64_t)k0 * lda + m0, lda, Kb - k0, M - m0, A, pt);
-        load_tile_kmajor<VECB>(Bs + st * kGBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, Kb - k0, N - n0, Bm, pt);
-        cp_async_mbar_arrive_noinc(full + st);
+        if (VECA == 2 && VECB == 2) {
+          // bulk-copy producers: warp 0 owns A, warp 1 owns B, the other two have nothing to do
+          if (pt < 64) {
+            mbar_wait(empty + st, ph);
+            if (pt < 32) bulk_load_tile_kmajor(As + st * kGBK * kLdT, A + (int64_t)k0 * lda + m0, lda, Kb - k0, M - m0, full + st, pt);
+            else bulk_load_tile_kmajor(Bs + st * kGBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, Kb - k0, N - n0, full + st, pt - 32);
+          }
+        } else {
+          mbar_wait(empty + st, ph);
+          load_tile_kmajor<VECA>(As + st * kGBK * kLdT, A + (int64_t)k0 * lda + m0, lda, Kb - k0, M - m0, A, pt);
+          load_tile_kmajor<VECB>(Bs + st * kGBK * kLdT, Bm + (int64_t)k0 * ldb + n0, ldb, Kb - k0, N - n0, Bm, pt);
+          cp_async_mbar_arrive_noinc(full + st);
+        }
         if (++st == kGemmStages) { st = 0; ph ^= 1; }
       }
     }
