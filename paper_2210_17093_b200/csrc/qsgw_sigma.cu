@@ -189,7 +189,8 @@ cudaError_t configure_kernels_for_device(int dev) {
   set(allow_smem(gemm_tn_dmma_kernel<1, 1, EpiStore>, kGemmSmemBytes));
   set(allow_smem(gemm_tn_dmma_kernel<2, 2, EpiPairScatter>, kGemmSmemBytes));
   set(allow_smem(gemm_tn_dmma_kernel<2, 2, EpiCasida>, kGemmSmemBytes));
-  set(allow_smem(sigma_accumulate_kernel, kSigmaSmemBudget + 1024));
+  set(allow_smem(sigma_accumulate_kernel<true>, kSigmaSmemBudget + 1024));
+  set(allow_smem(sigma_accumulate_kernel<false>, kSigmaSmemBudget + 1024));
   set(allow_smem(sigma_diag_kernel, kDiagSmemMax));
   if (e == cudaSuccess && dev >= 0 && dev < kMaxDevices) g_attr_done[dev] = true;
   return e;
@@ -324,7 +325,9 @@ int run_stage3(qsgw_sigma_plan *p, const double *WA, int64_t ldA, const double *
   if ((rc = encode_operand_map(p, &mapB, WB, ldB, sc, p->tq))) return rc;
   const SigmaRings rings = sigma_rings(p->tq);
   const int ntp = (p->n_mo + kTP - 1) / kTP;
-  sigma_accumulate_kernel<<<dim3(ntp * p->ntq, p->nsplit), kThreads, rings.smem_bytes, p->stream>>>(
+  // tiles of up to 224 columns (at most 7 column fragments per warp) take the instance with the hand-pipelined DMMA loop
+  auto kern = p->tq <= 224 ? sigma_accumulate_kernel<true> : sigma_accumulate_kernel<false>;
+  kern<<<dim3(ntp * p->ntq, p->nsplit), kThreads, rings.smem_bytes, p->stream>>>(
       mapA, mapB, p->eps, p->occ, Omega_c, p->n_mo, sc, p->eta * p->eta, p->nsplit, p->ntq, p->tq, rings.nA, rings.nB, p->Tpart);
   p->kernel_launches += 1;
   QSGW_CUDA(p, cudaGetLastError());

@@ -155,8 +155,8 @@ __device__ __forceinline__ void mbar_arrive_s(uint32_t bar) {
 // next step are fetched into the registers of this step as they fall free (a[i] after the DMMAs of row i, b[j] during
 // the last row); at the last step of a half the barrier waits of the next half come first.  The q-row stage of a half
 // is released as soon as that half is consumed; the p-row stage after both halves.
-template <int MI, int NJ>
-__device__ __forceinline__ void sigma_consumer_kloop(double (&acc)[4][8][2], const SigmaConsumerRings &r, uint32_t sw0, int KT, int lane) {
+template <int MI, int NJ, int NJM>
+__device__ __forceinline__ void sigma_consumer_kloop(double (&acc)[4][NJM][2], const SigmaConsumerRings &r, uint32_t sw0, int KT, int lane) {
   int sa = 0, sb = 0;
   uint32_t pha = 0, phb = 0;
   double a[MI], b[NJ];
@@ -217,47 +217,87 @@ __device__ __forceinline__ void sigma_consumer_kloop(double (&acc)[4][8][2], con
   }
 }
 
-template <int MI>
-__device__ __forceinline__ void sigma_consumer_kloop_nj(double (&acc)[4][8][2], const SigmaConsumerRings &r, uint32_t sw, int KT,
-                                                        int lane, int nj) {
-  switch (nj) {
-    case 1: sigma_consumer_kloop<MI, 1>(acc, r, sw, KT, lane); break;
-    case 2: sigma_consumer_kloop<MI, 2>(acc, r, sw, KT, lane); break;
-    case 3: sigma_consumer_kloop<MI, 3>(acc, r, sw, KT, lane); break;
-    case 4: sigma_consumer_kloop<MI, 4>(acc, r, sw, KT, lane); break;
-    case 5: sigma_consumer_kloop<MI, 5>(acc, r, sw, KT, lane); break;
-    case 6: sigma_consumer_kloop<MI, 6>(acc, r, sw, KT, lane); break;
-    case 7: sigma_consumer_kloop<MI, 7>(acc, r, sw, KT, lane); break;
-    default: sigma_consumer_kloop<MI, 8>(acc, r, sw, KT, lane); break;
+// One 16-pole half of a k-tile: acc[i][j] += A[p rows of fragment i][k] * Wq[q rows of fragment j][k], k = 0..15, for
+// the first MI x NJ fragments of the warp.  ap / bp: this lane's row (8 wmi + g resp. 8 wni + g) of the half, at byte
+// offset 8 (t & 1); sw[kk]: the lane's swizzled 16-byte chunk offset of k4 step kk.  Rows are 128 bytes; fragment i of
+// the p operand is 16 rows further, fragment j of the q operand 32 rows.  MI, NJ are compile-time: a predicated-off
+// DMMA still occupies the FP64 pipe for its full issue time, so ragged edge tiles BRANCH around unowned fragments.
+template <int MI, int NJ, int NJM>
+__device__ __forceinline__ void mma_half_sigma(double (&acc)[4][NJM][2], const char *ap, const char *bp, const int (&sw)[4]) {
+#pragma unroll
+  for (int kk = 0; kk < 4; ++kk) {
+    double a[MI], b[NJ];
+#pragma unroll
+    for (int i = 0; i < MI; ++i) a[i] = *reinterpret_cast<const double *>(ap + 16 * i * kHalfRowBytes + sw[kk]);
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) b[j] = *reinterpret_cast<const double *>(bp + 32 * j * kHalfRowBytes + sw[kk]);
+#pragma unroll
+    for (int i = 0; i < MI; ++i)
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) dmma_m8n8k4(acc[i][j], a[i], b[j]);
   }
 }
 
-// Ragged tile: dispatch (warp-uniform) on the fragment counts of this warp.  A warp without any fragment still walks the
-// rings: it owes the issuer its `empty` arrivals.
-__device__ __forceinline__ void sigma_consumer_kloop_ragged(double (&acc)[4][8][2], const SigmaConsumerRings &r, uint32_t sw,
-                                                            int KT, int lane, int mi, int nj) {
-  if (mi == 0 || nj == 0) {
-    int sa = 0, sb = 0;
-    uint32_t pha = 0, phb = 0;
-#pragma unroll 1
-    for (int kt = 0; kt < KT; ++kt) {
-      mbar_wait_s(r.a_full + 8 * sa, pha);
-      for (int h = 0; h < 2; ++h) {
-        mbar_wait_s(r.b_full + 8 * sb, phb);
-        __syncwarp();
-        if (lane == 0) mbar_arrive_s(r.b_empty + 8 * sb);
-        if (++sb == r.nB) { sb = 0; phb ^= 1; }
-      }
-      if (lane == 0) mbar_arrive_s(r.a_empty + 8 * sa);
-      if (++sa == r.nA) { sa = 0; pha ^= 1; }
-    }
-    return;
+template <int MI, int NJM>
+__device__ __forceinline__ void mma_half_sigma_nj(double (&acc)[4][NJM][2], const char *ap, const char *bp, const int (&sw)[4], int nj) {
+  switch (nj) {
+    case 1: if constexpr (NJM >= 1) mma_half_sigma<MI, 1>(acc, ap, bp, sw); break;
+    case 2: if constexpr (NJM >= 2) mma_half_sigma<MI, 2>(acc, ap, bp, sw); break;
+    case 3: if constexpr (NJM >= 3) mma_half_sigma<MI, 3>(acc, ap, bp, sw); break;
+    case 4: if constexpr (NJM >= 4) mma_half_sigma<MI, 4>(acc, ap, bp, sw); break;
+    case 5: if constexpr (NJM >= 5) mma_half_sigma<MI, 5>(acc, ap, bp, sw); break;
+    case 6: if constexpr (NJM >= 6) mma_half_sigma<MI, 6>(acc, ap, bp, sw); break;
+    case 7: if constexpr (NJM >= 7) mma_half_sigma<MI, 7>(acc, ap, bp, sw); break;
+    case 8: if constexpr (NJM >= 8) mma_half_sigma<MI, 8>(acc, ap, bp, sw); break;
+    default: break;
   }
+}
+
+// Ragged tile: dispatch (warp-uniform) on the fragment counts of this warp.
+template <int NJM>
+__device__ __forceinline__ void mma_half_sigma_ragged(double (&acc)[4][NJM][2], const char *ap, const char *bp, const int (&sw)[4],
+                                                      int mi, int nj) {
   switch (mi) {
-    case 1: sigma_consumer_kloop_nj<1>(acc, r, sw, KT, lane, nj); break;
-    case 2: sigma_consumer_kloop_nj<2>(acc, r, sw, KT, lane, nj); break;
-    case 3: sigma_consumer_kloop_nj<3>(acc, r, sw, KT, lane, nj); break;
-    default: sigma_consumer_kloop_nj<4>(acc, r, sw, KT, lane, nj); break;
+    case 1: mma_half_sigma_nj<1>(acc, ap, bp, sw, nj); break;
+    case 2: mma_half_sigma_nj<2>(acc, ap, bp, sw, nj); break;
+    case 3: mma_half_sigma_nj<3>(acc, ap, bp, sw, nj); break;
+    case 4: mma_half_sigma_nj<4>(acc, ap, bp, sw, nj); break;
+    default: break;
+  }
+}
+
+
+// The k loop for every other fragment count (256-column tiles with all 8 column fragments, the short last p row, narrow
+// last q-tiles): ONE loop with the (warp-uniform) dispatch on the fragment counts inside, barrier waits at the top of a
+// half.  With all 128 accumulator registers in use the hand-pipelined loop above spills ~20 doubles per k-tile (xl: 7891 vs
+// 7662 ms per build), and one loop per fragment-count pair makes ptxas spill in all of them, so only the hot
+// pairs of the small-to-large sizes (4 x 4..7) get the pipelined loop.
+template <int NJM>
+__device__ __forceinline__ void sigma_consumer_kloop_generic(double (&acc)[4][NJM][2], const char *a_ring, const char *b_ring,
+                                                             int b_stage_bytes, uint64_t *a_full, uint64_t *a_empty, uint64_t *b_full,
+                                                             uint64_t *b_empty, int nA, int nB, const int (&sw)[4], int KT, int lane,
+                                                             int mi, int nj) {
+  const bool full_tile = mi == 4 && nj == 8;
+  int sa = 0, sb = 0;
+  uint32_t pha = 0, phb = 0;
+#pragma unroll 1
+  for (int kt = 0; kt < KT; ++kt) {
+    mbar_wait(a_full + sa, pha);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      mbar_wait(b_full + sb, phb);
+      const char *ap = a_ring + sa * kAStageBytes + h * (kTP * kHalfRowBytes);
+      const char *bp = b_ring + (size_t)sb * b_stage_bytes;
+      if (NJM == 8 && full_tile) mma_half_sigma<4, NJM>(acc, ap, bp, sw);
+      else mma_half_sigma_ragged(acc, ap, bp, sw, mi, nj);
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(b_empty + sb);                 // this half of the q rows can be refilled while the other is in use
+        if (h) mbar_arrive(a_empty + sa);
+      }
+      if (++sb == nB) { sb = 0; phb ^= 1; }
+    }
+    if (++sa == nA) { sa = 0; pha ^= 1; }
   }
 }
 
@@ -269,6 +309,9 @@ __device__ __forceinline__ void sigma_consumer_kloop_ragged(double (&acc)[4][8][
 //   Omega [s_c]  excitation energies of the chunk
 //   Tpart [nsplit][N][N]  split-K partial tiles; slot z is owned by the CTAs of that slot and is
 //         read-modify-written once per launch -> accumulation order is fixed, results reproducible.
+// PIPE: the hand-pipelined DMMA loop for 4 x 4..7 fragments per warp (tiles of 104..224 columns); the host launches the
+// PIPE = false instance for wider tiles (all 8 column fragments in use, see sigma_consumer_kloop_generic).
+template <bool PIPE>
 __global__ void __launch_bounds__(kThreads, 1)
 sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
                         const double *__restrict__ eps, const double *__restrict__ occ, const double *__restrict__ Omega,
@@ -445,12 +488,12 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
     reg_inc<184>();
     const int cols_valid = min(tq, n_mo - q0);
     const SigmaFragMap fm(warp, lane, n_mo - p0, cols_valid);
-    const bool full_tile = fm.mi_cnt == 4 && fm.nj_cnt == 8;
-    double acc[4][8][2];
+    constexpr int NJM = PIPE ? 7 : 8;      // column fragments a warp can own: the accumulator registers follow
+    double acc[4][NJM][2];
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
-      for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+      for (int j = 0; j < NJM; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
     // 128-byte swizzle: 16-byte chunk c of row r lives at chunk c ^ (r & 7); every fragment row of this lane has
     // r & 7 == g.  Which of the 16 poles of a half a lane feeds into which k4 step is free as long as both operands agree
     // (the contraction sums over all of them), so lane t of step kk takes pole 8 (t >> 1) + 2 kk + (t & 1): chunk
@@ -459,15 +502,25 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
     const uint32_t sw = (uint32_t)(fm.g ^ ((fm.t >> 1) << 2)) << 4;   // k4 step kk reads chunk offset sw ^ (kk << 4)
     const int a_lane = (8 * fm.wmi + fm.g) * kHalfRowBytes + 8 * (fm.t & 1);
     const int b_lane = (8 * fm.wni + fm.g) * kHalfRowBytes + 8 * (fm.t & 1);
-    SigmaConsumerRings rings;
-    rings.a_ring = smem_u32(a_ring) + a_lane;
-    rings.b_ring = smem_u32(b_ring) + b_lane;
-    rings.a_full = smem_u32(a_full); rings.a_empty = smem_u32(a_empty);
-    rings.b_full = smem_u32(b_full); rings.b_empty = smem_u32(b_empty);
-    rings.nA = nA; rings.nB = nB; rings.b_stage_bytes = b_stage_bytes;
     if (KT > 0) {
-      if (full_tile) sigma_consumer_kloop<4, 8>(acc, rings, sw, KT, lane);
-      else sigma_consumer_kloop_ragged(acc, rings, sw, KT, lane, fm.mi_cnt, fm.nj_cnt);
+      if (PIPE && fm.mi_cnt == 4 && fm.nj_cnt >= 4 && fm.nj_cnt <= 7) {
+        SigmaConsumerRings rings;
+        rings.a_ring = smem_u32(a_ring) + a_lane;
+        rings.b_ring = smem_u32(b_ring) + b_lane;
+        rings.a_full = smem_u32(a_full); rings.a_empty = smem_u32(a_empty);
+        rings.b_full = smem_u32(b_full); rings.b_empty = smem_u32(b_empty);
+        rings.nA = nA; rings.nB = nB; rings.b_stage_bytes = b_stage_bytes;
+        if (fm.nj_cnt == 7) sigma_consumer_kloop<4, 7>(acc, rings, sw, KT, lane);
+        else if (fm.nj_cnt == 6) sigma_consumer_kloop<4, 6>(acc, rings, sw, KT, lane);
+        else if (fm.nj_cnt == 5) sigma_consumer_kloop<4, 5>(acc, rings, sw, KT, lane);
+        else sigma_consumer_kloop<4, 4>(acc, rings, sw, KT, lane);
+      } else {
+        int swk[4];
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) swk[kk] = (int)(sw ^ (kk << 4));
+        sigma_consumer_kloop_generic(acc, reinterpret_cast<const char *>(a_ring) + a_lane, reinterpret_cast<const char *>(b_ring) + b_lane,
+                                     b_stage_bytes, a_full, a_empty, b_full, b_empty, nA, nB, swk, KT, lane, fm.mi_cnt, fm.nj_cnt);
+      }
     }
 
     double *Tz = Tpart + (int64_t)z * n_mo * n_mo;
@@ -477,7 +530,7 @@ sigma_accumulate_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_c
       const int p = p0 + fm.row(i);
       if (p < n_mo) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        for (int j = 0; j < NJM; ++j) {
           const int qc = fm.out_col(j);
           const int q = q0 + qc;
           if (qc < cols_valid) {
