@@ -41,7 +41,10 @@ UNIT = "TFLOP/s"
 FP64_FMA_PER_CLK_PER_SM = 64
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE stage-2 launch over a full s-block, from committed `ncu --set full`
 # summaries (recorded numbers, not measurements of this run; the JSON line names the file)
-NCU_STAGE2_DRAM_BYTES_PER_LAUNCH = {}
+NCU_STAGE2_DRAM_BYTES_PER_LAUNCH = {
+    "xl": (196.99e9, "profiles/r02_full_xl.md"),          # 164.22 GB read + 32.77 GB written
+    "large": (29.95e9, "profiles/r02_full_large.md"),    # 18.17 GB read + 11.78 GB written
+}
 
 
 def pole_range(cfg) -> int:
@@ -376,7 +379,7 @@ def run_gpu(args):
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "launches": stats["launches_stage2"], "avg_launch_ms": s2_ms,
                          "traffic": traffic[0] if traffic else None,
-                         "traffic_source": (f"recorded: dram read + write bytes of one launch over a full s-block, ncu --set full, {traffic[1]}"
+                         "traffic_source": (f"recorded: dram read + write bytes of one launch over a full s-block, ncu, {traffic[1]}"
                                             if traffic else "no committed ncu capture for this workload"),
                          "peak_source": f"FP64 pipe rate at max SM clock ({peak_src} MEASURED_PEAKS.json sm_max_mhz; no FP64 entry is "
                                         "measured there); cross-checked in this run, see fp64_peak_tflops.in_run_checks"},

@@ -288,17 +288,26 @@ struct EpiPairScatter {
 };
 
 // Tile t of a batch -> (tm, tn).  tri: only the tiles with tm <= tn of a square tile grid are enumerated (symmetric
-// products: t = tn (tn + 1) / 2 + tm); otherwise all ntm x ntn tiles, the index named by m_fastest varying fastest.
+// products: t = tn (tn + 1) / 2 + tm); otherwise all ntm x ntn tiles.  m_fastest > 0: tm varies fastest; 0: tn varies
+// fastest; < 0: L2-aware order for many row tiles and few column tiles -- the column tiles are taken in groups of
+// g = -m_fastest whose B panels (g x K x 128 doubles) fit in L2 together, and inside a group tn varies fastest, so the
+// group's B panels stay resident while the A panels stream through once per group.
 __device__ __forceinline__ void decode_tile(int t, int ntm, int ntn, int m_fastest, int tri, int &tm, int &tn) {
   if (tri) {
     tn = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
     while (tn * (tn + 1) / 2 > t) --tn;
     while ((tn + 1) * (tn + 2) / 2 <= t) ++tn;
     tm = t - tn * (tn + 1) / 2;
-  } else if (m_fastest) {
+  } else if (m_fastest > 0) {
     tn = t / ntm; tm = t - tn * ntm;
-  } else {
+  } else if (m_fastest == 0) {
     tm = t / ntn; tn = t - tm * ntn;
+  } else {
+    const int g = -m_fastest, per_group = ntm * g;
+    const int grp = t / per_group, r = t - grp * per_group;
+    const int gsz = min(g, ntn - grp * g);
+    tm = r / gsz;
+    tn = grp * g + (r - tm * gsz);
   }
 }
 

@@ -220,8 +220,21 @@ int launch_gemm_on(qsgw_sigma_plan *p, cudaStream_t stream, int num_sms, const d
   if ((int64_t)ntm * ntn * nbatch > INT32_MAX) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "GEMM grid too large");
   // persistent: one CTA per SM walks the tiles round-robin; the dimension with fewer tiles varies fastest, so that the
   // CTAs running at the same time share its few operand panels in L2
+  // tile order: the dimension with fewer tiles varies fastest.  Many row tiles against few column tiles (stage 2): if the B
+  // panels of all column tiles do not fit in ~40 MB of L2, the column tiles are taken in groups that do (dmma_gemm.cuh,
+  // decode_tile), so that the A panels are re-read once per group instead of once per wave of CTAs.
+  int order = ntm <= ntn ? 1 : 0;
+  if (order == 0 && nbatch == 1 && ntn > 1) {
+    const double panel_bytes = 8.0 * (double)K * kBN;
+    int g = (int)std::max(1.0, std::floor(40e6 / panel_bytes));
+    if (g < ntn) {
+      const int groups = (ntn + g - 1) / g;
+      g = (ntn + groups - 1) / groups;            // equal groups
+      order = -g;
+    }
+  }
   kern<<<std::min(ntm * ntn * nbatch, num_sms), kThreads, kGemmSmemBytes, stream>>>(
-      A, lda, Bm, ldb, M, N, K, ntm, ntn, ntm <= ntn ? 1 : 0, nbatch, strideA, strideB, k_total, 0, epi);
+      A, lda, Bm, ldb, M, N, K, ntm, ntn, order, nbatch, strideA, strideB, k_total, 0, epi);
   QSGW_CUDA(p, cudaGetLastError());
   return QSGW_SIGMA_OK;
 }

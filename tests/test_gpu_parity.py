@@ -62,6 +62,8 @@ RAGGED = [
     (130, 3, 17, 381, 128),
     (131, 64, 33, 150, 0),
     (257, 5, 40, 300, 100),
+    (250, 20, 40, 200, 64),      # one 256-column q-tile: the stage-3 instance for 8 column fragments per warp
+    (233, 9, 24, 130, 0),        # the same instance with 8 / 8 / 7 / 7 column fragments
     (24, 23, 9, 23, 0),
     (2, 1, 1, 1, 0),
 ]
