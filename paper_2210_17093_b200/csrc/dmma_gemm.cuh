@@ -5,7 +5,8 @@
 // registers.  A CTA is 12 warps: 8 consumer warps (2 x 4, each a 64 x 32 warp tile of 8 x 4 DMMA fragments,
 // fragments interleaved across warps so that ragged edge tiles shed work evenly) that do nothing but
 // LDS.64 fragment loads + DMMA, and 4 producer warps (one per SM sub-partition) that stage the operand tiles
-// global -> shared with cp.async (LDGSTS).  The two roles meet only through mbarriers (full[stage] /
+// global -> shared: with cp.async.bulk row copies of the TMA unit when both operands are 16-byte aligned (two of the
+// warps, one lane per k-row), with 8 / 16-byte cp.async (LDGSTS) otherwise.  The two roles meet only through mbarriers (full[stage] /
 // empty[stage]); there is no CTA-wide barrier in the main loop, so the DMMA pipe never drains at a k-tile edge.
 // Registers are re-split with setmaxnreg (consumers up, producers down).  Shared tiles are padded so that every
 // fragment load is bank-conflict free.

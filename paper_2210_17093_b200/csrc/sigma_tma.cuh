@@ -17,7 +17,9 @@
 //     16-pole halves of a k-tile (a half is released, and its refill issued, as soon as it has been consumed);
 //   * 8 consumer warps (2 x 4) run LDS.64 fragment loads + DMMA.8x8x4 only, software-pipelined across k4 steps and ring
 //     stages (the next fragments, barrier waits included, are fetched under the current DMMAs); accumulators in registers;
-//   * split-K over m into slot-owned partial tiles (fixed accumulation order, no atomics).
+//   * split-K over a linear (m, 32-pole group) index into slot-owned partial tiles (fixed accumulation order, no atomics);
+//   * two instances: <true> for tiles of up to 224 columns (at most 7 column fragments per warp: 112 accumulator
+//     registers, hand-pipelined DMMA loop), <false> for 256-column tiles (all 128 accumulator registers, plain loop).
 #pragma once
 #include <cuda.h>
 
