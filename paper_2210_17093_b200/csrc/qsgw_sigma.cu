@@ -266,7 +266,8 @@ int do_begin(qsgw_sigma_plan *p, const double *B, const double *eps, const doubl
   p->B = B; p->eps = eps; p->occ = occ; p->eta = eta;
   {
     ScopedTimer t(p, kPack);
-    pack_pairs_kernel<<<dim3(p->n_mo, p->n_aux), 128, 0, p->stream>>>(B, p->n_mo, p->Bp, p->ldp);
+    pack_pairs_kernel<<<dim3((unsigned)((p->n_pair + kPackPairsPerBlock - 1) / kPackPairsPerBlock), p->n_aux), 256, 0, p->stream>>>(
+        B, p->pairs, p->n_mo, p->n_pair, p->Bp, p->ldp);
     p->kernel_launches += 2;
     QSGW_CUDA(p, cudaGetLastError());
     dim3 grid((p->n_virt + 31) / 32, (p->n_aux + 31) / 32, p->n_occ);

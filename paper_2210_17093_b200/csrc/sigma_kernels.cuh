@@ -14,11 +14,24 @@ __host__ __device__ __forceinline__ int64_t pair_offset(int p, int n_mo) {
 
 // Bp[P][r(p,m)] = B[P][p][m] for p <= m: the A operand of stage 2 with the p<->m symmetry of
 // w (B^P_pm = B^P_mp, real orbitals) folded in, so stage 2 does N(N+1)/2 rows, not N^2.
-__global__ void pack_pairs_kernel(const double *__restrict__ B, int n_mo, double *__restrict__ Bp, int64_t ldp) {
-  const int p = blockIdx.x, P = blockIdx.y;
-  const double *src = B + ((int64_t)P * n_mo + p) * n_mo;
-  double *dst = Bp + (int64_t)P * ldp + pair_offset(p, n_mo) - p;
-  for (int m = p + threadIdx.x; m < n_mo; m += blockDim.x) dst[m] = src[m];
+// One thread per pair and auxiliary function (4 pairs per thread): the pair table gives (p, m), consecutive pairs of a row p
+// are consecutive m, so reads and writes are coalesced, and a small N (the paper's molecules) still fills its blocks.
+constexpr int kPackPairsPerBlock = 1024;
+__global__ void __launch_bounds__(256)
+pack_pairs_kernel(const double *__restrict__ B, const int2 *__restrict__ pairs, int n_mo, int64_t n_pair, double *__restrict__ Bp,
+                  int64_t ldp) {
+  const int P = blockIdx.y;
+  const double *src = B + (int64_t)P * n_mo * n_mo;
+  double *dst = Bp + (int64_t)P * ldp;
+  const int64_t r0 = (int64_t)blockIdx.x * kPackPairsPerBlock + threadIdx.x;
+#pragma unroll
+  for (int k = 0; k < kPackPairsPerBlock / 256; ++k) {
+    const int64_t r = r0 + k * 256;
+    if (r < n_pair) {
+      const int2 pm = __ldg(pairs + r);
+      dst[r] = __ldg(src + (int64_t)pm.x * n_mo + pm.y);
+    }
+  }
 }
 
 __global__ void pair_table_kernel(int n_mo, int2 *__restrict__ pairs) {
