@@ -200,6 +200,22 @@ int qsgw_ri_ao_to_mo(const double *B_ao, const double *C, int n_aux, int n_ao, i
 size_t qsgw_ri_ao_to_mo_work_doubles(int n_aux, int n_ao, int n_mo);
 
 /*
+ * The same transformation for callers that must not allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc) and have no scratch buffer of their own: the `work` array of qsgw_ri_ao_to_mo is a
+ * file-scope device array of the library, qsgw_ri_ao_to_mo_static_max_doubles() = 8 Mi doubles = 64 MiB, which every GPU
+ * that loads the library holds until the process exits.  The call allocates nothing (no cudaMalloc / cudaFree, no allocating
+ * library routine); arguments, layouts, results and asynchrony are those of qsgw_ri_ao_to_mo.
+ *   - Limit: n_aux * n_ao * round_up(n_mo, 2) <= 8 Mi doubles (e.g. the `small` config, 400 x 120 x 120); larger problems
+ *     return INVALID_ARG with a message that names the limit -- use qsgw_ri_ao_to_mo with a caller-owned buffer.
+ *   - ALL calls on one GPU share the one array, which keeps the contents of the last call (nothing in it has to start at
+ *     zero).  Two calls that overlap on the GPU -- different streams, or different host threads on different streams -- RACE
+ *     on it and give wrong results; calls on one stream are ordered and safe.
+ * Errors: as qsgw_ri_ao_to_mo; CUDA also if the address of the array cannot be obtained on the current device.
+ */
+int qsgw_ri_ao_to_mo_static(const double *B_ao, const double *C, int n_aux, int n_ao, int n_mo, double *B_mo, void *cuda_stream);
+size_t qsgw_ri_ao_to_mo_static_max_doubles(void);
+
+/*
  * Row 8(e) / 8(f).4 of the scope table: the build shards over the pole index s.  Sigma is a plain sum over s (Eq. (17),
  * PAPER.md:149), V[:,s] depends only on Z[:,s] and w^s only on V[:,s], so rank r of n_ranks runs
  * qsgw_sigma_begin / _add_poles / _finish on the contiguous slice Omega[s0 .. s0+n), Z[:, s0 .. s0+n) of the poles (B, eps,

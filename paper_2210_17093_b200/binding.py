@@ -27,7 +27,7 @@ QSGW_SIGMA_ERR_CUDA = -3
 
 EXPORTS = (
     "qsgw_sigma_create", "qsgw_sigma_build", "qsgw_sigma_begin", "qsgw_sigma_add_poles", "qsgw_sigma_finish",
-    "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_mp2_direct_build", "qsgw_mp2_build", "qsgw_ri_ao_to_mo", "qsgw_ri_ao_to_mo_work_doubles", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
+    "qsgw_sigma_build_host", "qsgw_sigma_diag_build", "qsgw_mp2_direct_build", "qsgw_mp2_build", "qsgw_ri_ao_to_mo", "qsgw_ri_ao_to_mo_work_doubles", "qsgw_ri_ao_to_mo_static", "qsgw_ri_ao_to_mo_static_max_doubles", "qsgw_sigma_destroy", "qsgw_sigma_last_error", "qsgw_sigma_workspace_bytes",
     "qsgw_sigma_limit_pole_batch", "qsgw_sigma_set_profiling", "qsgw_sigma_get_stats", "qsgw_sigma_set_debug", "qsgw_sigma_version",
     "qsgw_sigma_pole_slice", "qsgw_casida_work_doubles", "qsgw_casida_matrix", "qsgw_casida_z",
 )
@@ -89,6 +89,10 @@ def load_library() -> ctypes.CDLL:
         lib.qsgw_ri_ao_to_mo.argtypes = [dp, dp, ci, ci, ci, dp, dp, vp]
         lib.qsgw_ri_ao_to_mo_work_doubles.restype = ctypes.c_size_t
         lib.qsgw_ri_ao_to_mo_work_doubles.argtypes = [ci, ci, ci]
+        lib.qsgw_ri_ao_to_mo_static.restype = ci
+        lib.qsgw_ri_ao_to_mo_static.argtypes = [dp, dp, ci, ci, ci, dp, vp]
+        lib.qsgw_ri_ao_to_mo_static_max_doubles.restype = ctypes.c_size_t
+        lib.qsgw_ri_ao_to_mo_static_max_doubles.argtypes = []
         lib.qsgw_sigma_destroy.restype = ci
         lib.qsgw_sigma_destroy.argtypes = [vp]
         lib.qsgw_sigma_last_error.restype = ctypes.c_char_p
@@ -276,6 +280,27 @@ def qsgw_mp2_build(plan: Plan, B, eps, occ, eta: float, Sigma: Optional[torch.Te
 
 def qsgw_ri_ao_to_mo_work_doubles(n_aux: int, n_ao: int, n_mo: int) -> int:
     return int(load_library().qsgw_ri_ao_to_mo_work_doubles(int(n_aux), int(n_ao), int(n_mo)))
+
+
+def qsgw_ri_ao_to_mo_static_max_doubles() -> int:
+    return int(load_library().qsgw_ri_ao_to_mo_static_max_doubles())
+
+
+def qsgw_ri_ao_to_mo_static(B_ao: torch.Tensor, C: torch.Tensor, B_mo: torch.Tensor,
+                            stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """qsgw_ri_ao_to_mo with the library's static scratch array: the call allocates nothing, so B_mo is the caller's.
+    Calls that overlap on the GPU race on the shared scratch (include/qsgw_sigma.h)."""
+    if B_ao.dim() != 3 or B_ao.shape[1] != B_ao.shape[2] or C.dim() != 2 or C.shape[0] != B_ao.shape[1]:
+        raise ValueError("need B_ao [n_aux, n_ao, n_ao] and C [n_ao, n_mo]")
+    if not B_ao.is_contiguous() or not C.is_contiguous():
+        raise ValueError("B_ao and C must be contiguous")
+    n_aux, n_ao, n_mo = int(B_ao.shape[0]), int(B_ao.shape[1]), int(C.shape[1])
+    if stream is None:
+        stream = torch.cuda.current_stream(B_ao.device)
+    rc = load_library().qsgw_ri_ao_to_mo_static(_dev(B_ao, "B_ao"), _dev(C, "C"), n_aux, n_ao, n_mo,
+                                                _dev(B_mo, "B_mo", (n_aux, n_mo, n_mo)), ctypes.c_void_p(stream.cuda_stream))
+    _check(rc, None)
+    return B_mo
 
 
 def qsgw_ri_ao_to_mo(B_ao: torch.Tensor, C: torch.Tensor, B_mo: Optional[torch.Tensor] = None,

@@ -173,6 +173,28 @@ constexpr int kMaxDevices = 64;
 std::mutex g_attr_mutex;
 bool g_attr_done[kMaxDevices] = {};
 
+// Scratch of qsgw_ri_ao_to_mo_static: a file-scope device array, so that entry point never allocates.  Every GPU that loads
+// the library holds these 64 MiB until the process exits.  In HOST code the name below is a host-side stand-in, not a device
+// address; the address a kernel may use comes from cudaGetSymbolAddress, looked up once per device with that device current.
+constexpr size_t kStaticWorkDoubles = (size_t)8 << 20;      // 8 Mi doubles = 64 MiB
+static __device__ __align__(256) double g_aomo_static_work[kStaticWorkDoubles];
+double *g_aomo_static_ptr[kMaxDevices] = {};
+
+// device address of g_aomo_static_work on the CURRENT device `dev`
+cudaError_t static_work_address(int dev, double **ptr) {
+  std::lock_guard<std::mutex> lock(g_attr_mutex);
+  if (dev >= 0 && dev < kMaxDevices && g_aomo_static_ptr[dev]) {
+    *ptr = g_aomo_static_ptr[dev];
+    return cudaSuccess;
+  }
+  double *addr = nullptr;
+  cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void **>(&addr), g_aomo_static_work);
+  if (e != cudaSuccess) return e;
+  if (dev >= 0 && dev < kMaxDevices) g_aomo_static_ptr[dev] = addr;
+  *ptr = addr;
+  return cudaSuccess;
+}
+
 template <class Kern>
 cudaError_t allow_smem(Kern kern, size_t bytes) {
   return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -935,6 +957,32 @@ int qsgw_ri_ao_to_mo(const double *B_ao, const double *C, int n_aux, int n_ao, i
     if (rc) return rc;
   }
   return QSGW_SIGMA_OK;
+}
+
+size_t qsgw_ri_ao_to_mo_static_max_doubles(void) { return kStaticWorkDoubles; }
+
+int qsgw_ri_ao_to_mo_static(const double *B_ao, const double *C, int n_aux, int n_ao, int n_mo, double *B_mo, void *cuda_stream) {
+  if (n_aux < 1 || n_ao < 1 || n_mo < 1) return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, "ao_to_mo_static: sizes must be >= 1");
+  const size_t need = qsgw_ri_ao_to_mo_work_doubles(n_aux, n_ao, n_mo);
+  if (need > kStaticWorkDoubles) {
+    char buf[256];
+    snprintf(buf, sizeof buf,
+             "ao_to_mo_static: n_aux * n_ao * round_up(n_mo, 2) = %zu doubles of scratch exceed the static maximum of %zu (64 MiB); "
+             "use qsgw_ri_ao_to_mo with a caller-owned work buffer",
+             need, (size_t)kStaticWorkDoubles);
+    return fail(nullptr, QSGW_SIGMA_ERR_INVALID_ARG, buf);
+  }
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  double *work = nullptr;
+  if (e == cudaSuccess) e = static_work_address(dev, &work);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, QSGW_SIGMA_ERR_CUDA, std::string("ao_to_mo_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+  }
+  // Nothing in the scratch has to start at zero: the first GEMM overwrites every element whose value reaches an output of
+  // the second (the padding column of an odd n_mo only feeds accumulator columns that are never stored).
+  return qsgw_ri_ao_to_mo(B_ao, C, n_aux, n_ao, n_mo, work, B_mo, cuda_stream);
 }
 
 size_t qsgw_casida_work_doubles(int n_mo, int n_occ, int n_aux) {
