@@ -127,8 +127,9 @@ int qsgw_sigma_finish(qsgw_sigma_plan *plan, double *Sigma);
 
 /*
  * Same build with HOST buffers (same shapes and meaning as qsgw_sigma_build): the library uploads
- * B, eps, occ once and Omega/Z in ranges of one s_block of poles, overlapping the upload of the
- * next range with the kernels of the current one, downloads Sigma and synchronises before returning.
+ * B, eps, occ once and Omega/Z in ranges of poles (the first of one s_block, the later ones of up to four
+ * s_blocks, at most 6 GB of Z each), overlapping the upload of the next range with the kernels of the
+ * current one, downloads Sigma and synchronises before returning.
  * n_pole may exceed n_pole_max.  Device staging buffers for the host path are allocated on the first
  * call (not in create) and kept by the plan; ALLOC if they do not fit.
  * Of B only the entries B[P][p][q] with p <= q are read (and uploaded): B is symmetric in its last two

@@ -517,12 +517,24 @@ int do_finish(qsgw_sigma_plan *p, double *Sigma) {
   return QSGW_SIGMA_OK;
 }
 
+// Poles per uploaded range of the host path (the first range of a build is one s-block, so that compute starts early).
+// Every range launches its own stage 1; with one s-block per range that GEMM has too few tiles for the 148 SMs (large:
+// 608 tiles = 4.1 waves, a fifth of stage 1 lost to the last wave), so later ranges take up to 4 s-blocks -- as many as
+// fit in 6 GB per Z buffer and in the V workspace.
+int64_t host_range(const qsgw_sigma_plan *p) {
+  const double chunk_bytes = 8.0 * (double)p->n_ov * p->s_chunk;
+  int64_t k = (int64_t)std::floor(6e9 / chunk_bytes);
+  k = std::max<int64_t>(1, std::min<int64_t>(4, k));
+  k = std::max<int64_t>(1, std::min<int64_t>(k, p->v_cols_alloc / p->s_chunk));
+  return k * p->s_chunk;
+}
+
 void free_host_staging(qsgw_sigma_plan *p) {
   auto release = [&](double *&ptr, size_t count) {
     if (ptr) { cudaFree(ptr); p->bytes -= std::max<size_t>(count, 1) * sizeof(double); ptr = nullptr; }
   };
   const size_t nn = (size_t)p->n_mo * p->n_mo;
-  const int64_t ld = round_up(p->s_chunk, 2);
+  const int64_t ld = round_up(host_range(p), 2);
   release(p->hB, (size_t)p->n_aux * nn);
   release(p->hEps, p->n_mo);
   release(p->hOcc, p->n_mo);
@@ -543,7 +555,7 @@ void free_host_staging(qsgw_sigma_plan *p) {
 // allocation fails the partial ones are released again, so a later call starts from scratch.
 int ensure_host_staging(qsgw_sigma_plan *p) {
   if (p->staging_ready) return QSGW_SIGMA_OK;
-  const int64_t range = p->s_chunk;   // one w chunk per uploaded pole range
+  const int64_t range = host_range(p);
   const size_t nn = (size_t)p->n_mo * p->n_mo;
   const int64_t ld = round_up(range, 2);
   int rc = QSGW_SIGMA_OK;
@@ -838,7 +850,7 @@ int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps
   if (n_pole < 1 || ldz < n_pole) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build_host: need 1 <= n_pole <= ldz");
   if (!(eta > 0.0)) return fail(p, QSGW_SIGMA_ERR_INVALID_ARG, "build_host: eta must be > 0");
   if ((rc = ensure_host_staging(p))) return rc;
-  const int64_t R = p->h_range, ldr = round_up(R, 2);
+  const int64_t R = std::min<int64_t>(p->h_range, p->n_pole_max), ldr = round_up(R, 2);   // add_poles takes at most n_pole_max
   const size_t nn = (size_t)p->n_mo * p->n_mo;
 
   // B, eps, occ on the compute stream (begin needs them first).  The build reads B[P][p][q] only for p <= q (B is symmetric
@@ -864,8 +876,7 @@ int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps
   QSGW_CUDA(p, cudaMemcpyAsync(p->hOcc, occ, sizeof(double) * p->n_mo, cudaMemcpyHostToDevice, p->stream));
 
   // pole ranges: upload range r+1 on the copy stream while the compute stream works on range r
-  auto upload = [&](int64_t s0, int buf) -> int {
-    const int64_t n = std::min<int64_t>(R, n_pole - s0);
+  auto upload = [&](int64_t s0, int64_t n, int buf) -> int {
     QSGW_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->ev_consumed[buf], 0));
     QSGW_CUDA(p, cudaMemcpyAsync(p->hOmega[buf], Omega + s0, sizeof(double) * n, cudaMemcpyHostToDevice, p->copy_stream));
     QSGW_CUDA(p, cudaMemcpy2DAsync(p->hZ[buf], sizeof(double) * ldr, Z + s0, sizeof(double) * ldz, sizeof(double) * n,
@@ -876,12 +887,14 @@ int qsgw_sigma_build_host(qsgw_sigma_plan *p, const double *B, const double *eps
   // both buffers start out free
   QSGW_CUDA(p, cudaEventRecord(p->ev_consumed[0], p->stream));
   QSGW_CUDA(p, cudaEventRecord(p->ev_consumed[1], p->stream));
-  if ((rc = upload(0, 0))) return rc;
+  // ranges: one s-block first, then R poles each
+  const int64_t n_first = std::min<int64_t>(p->s_chunk, n_pole);
+  if ((rc = upload(0, n_first, 0))) return rc;
   if ((rc = do_begin(p, p->hB, p->hEps, p->hOcc, eta))) return rc;
   int buf = 0;
-  for (int64_t s0 = 0; s0 < n_pole; s0 += R, buf ^= 1) {
-    const int64_t n = std::min<int64_t>(R, n_pole - s0);
-    if (s0 + R < n_pole && (rc = upload(s0 + R, buf ^ 1))) { p->begun = false; return rc; }
+  for (int64_t s0 = 0, n = n_first; s0 < n_pole; s0 += n, n = std::min<int64_t>(R, n_pole - s0), buf ^= 1) {
+    const int64_t s_next = s0 + n;
+    if (s_next < n_pole && (rc = upload(s_next, std::min<int64_t>(R, n_pole - s_next), buf ^ 1))) { p->begun = false; return rc; }
     QSGW_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_copied[buf], 0));
     if ((rc = do_add_poles(p, p->hOmega[buf], p->hZ[buf], ldr, n))) { p->begun = false; return rc; }
     QSGW_CUDA(p, cudaEventRecord(p->ev_consumed[buf], p->stream));

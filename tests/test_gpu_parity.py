@@ -190,6 +190,20 @@ def test_host_buffer_entry_point_matches_device_entry_point():
     pkg.qsgw_sigma_destroy(plan)
 
 
+def test_host_buffer_entry_point_with_more_poles_than_the_plan_capacity_and_unequal_ranges():
+    """n_pole > n_pole_max through the host path: the library uploads one s-block first and then ranges of four s-blocks
+    (64, 256 and 220 poles here), each with its own stage 1; compared with the oracle, and twice for reproducibility."""
+    pkg = _pkg()
+    cfg = qi.custom_config(70, 9, 45, n_pole=540, s_block=64, seed=23)
+    inp = qi.make_inputs(cfg)
+    plan = pkg.qsgw_sigma_create(cfg.n_mo, cfg.n_occ, cfg.n_aux, 256, cfg.s_block)
+    S1 = pkg.qsgw_sigma_build_host(plan, inp.B, inp.eps, inp.occ, inp.Omega, inp.Z, cfg.eta)
+    S2 = pkg.qsgw_sigma_build_host(plan, inp.B, inp.eps, inp.occ, inp.Omega, inp.Z, cfg.eta)
+    assert torch.equal(S1, S2) and torch.equal(S1, S1.T)
+    _assert_parity(S1, _ref_sigma(cfg, inp))
+    pkg.qsgw_sigma_destroy(plan)
+
+
 def test_null_case_and_error_codes():
     pkg = _pkg()
     cfg = qi.CONFIGS["tiny"]
